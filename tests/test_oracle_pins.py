@@ -1,0 +1,339 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these retype the oracle's formulas: each compares the oracle with a closed form, an invariant,
+a dense-matrix brute force built here with numpy, or a library routine (numpy.fft, scipy.linalg.expm).
+"""
+import os
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+from paper_1204_5434_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ FFT ----------
+@pytest.mark.parametrize("n", [1, 2, 4, 6, 8, 15, 16, 32, 64])
+def test_fft_matches_definition_and_numpy(oracle, n):
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    X = oracle.fft1d(x, -1)
+    assert np.max(np.abs(X - oracle.dft1d_direct(x, -1))) < 1e-13 * n
+    assert np.max(np.abs(X - np.fft.fft(x))) < 1e-13 * n                       # sign convention e^{-ikx}
+    assert np.max(np.abs(oracle.fft1d(X, +1) - x)) < 1e-13                     # F^-1 F = I, 1/n on the inverse
+    assert abs(np.sum(np.abs(X) ** 2) / n - np.sum(np.abs(x) ** 2)) < 1e-12 * n   # Parseval
+
+
+# ------------------------------------------------------------------ uniform field ---------------
+@pytest.mark.parametrize("w0", [0.7, 0.3 - 1.1j])
+def test_uniform_field_closed_form(oracle, w0):
+    """q_j = exp(-w0 j ds), Q = exp(-w0), phi = 1 (north_star; closed form of PAPER.md Eq. 4-5)."""
+    grid, Ns = (4, 8, 2), 16
+    o = oracle.Oracle(grid, (3.0, 4.0, 5.0), Ns, "external")
+    o.set_fields(np.full(grid, w0, np.complex128))
+    o.propagate()
+    Q, phi, _ = o.density_operators()
+    assert abs(Q - np.exp(-w0)) < 1e-14
+    assert np.max(np.abs(phi - 1.0)) < 1e-13
+    for j in (0, 1, 7, Ns):
+        assert np.max(np.abs(o.get_slice(0, j) - np.exp(-w0 * j / Ns))) < 1e-14
+
+
+def test_uniform_diblock_closed_form(oracle):
+    grid, Ns, fA = (4, 4, 4), 20, 0.3
+    wp, wm = 0.4 + 0.2j, -0.6 + 0.1j
+    o = oracle.Oracle(grid, (4.0, 4.0, 4.0), Ns, "diblock", fA=fA, chiN=15.0)
+    o.set_fields(np.full(grid, wp, np.complex128), np.full(grid, wm, np.complex128))
+    o.propagate()
+    Q, pa, pb = o.density_operators()
+    wA, wB = wp - wm, wp + wm
+    assert abs(Q - np.exp(-(fA * wA + (1 - fA) * wB))) < 1e-14
+    assert np.max(np.abs(pa - fA)) < 1e-13 and np.max(np.abs(pb - (1 - fA))) < 1e-13
+
+
+# ------------------------------------------------------------------ dense brute force -----------
+def _dense_dft(n):
+    k = np.arange(n)
+    return np.exp(-2j * np.pi * np.outer(k, k) / n)
+
+
+def _dense_k2(grid, cell):
+    ks = []
+    for n, L in zip(grid, cell):
+        i = np.arange(n)
+        ks.append(2 * np.pi * np.where(i <= n // 2, i, i - n) / L)
+    KX, KY, KZ = np.meshgrid(*ks, indexing="ij")
+    return (KX ** 2 + KY ** 2 + KZ ** 2).ravel()
+
+
+def _dense_F(grid):
+    return np.kron(np.kron(_dense_dft(grid[0]), _dense_dft(grid[1])), _dense_dft(grid[2]))
+
+
+@pytest.mark.parametrize("grid,cell", [((4, 4, 4), (3.0, 4.0, 5.0)), ((2, 8, 4), (2.0, 6.0, 3.5))])
+def test_rqm4_step_equals_dense_operator(oracle, grid, cell):
+    """Eq. 12 multiplied out as dense M x M matrices."""
+    M = int(np.prod(grid))
+    ds = 0.05
+    w = inputs.random_complex_field(grid, 1, scale=0.8, mean=0.3).ravel()
+    q = (1.0 + inputs.random_complex_field(grid, 2, scale=0.5)).ravel()
+    F = _dense_F(grid)
+    Fi = np.conj(F).T / M
+    k2 = _dense_k2(grid, cell)
+    D = lambda a: Fi @ np.diag(np.exp(-a * k2 * ds)) @ F
+    E = lambda a: np.diag(np.exp(-a * w * ds))
+    full = E(0.5) @ D(1.0) @ E(0.5)
+    half = E(0.25) @ D(0.5) @ E(0.5) @ D(0.5) @ E(0.25)
+    U = (4.0 * half - full) / 3.0
+    got = oracle.rqm4_step(grid, cell, ds, w.reshape(grid), q.reshape(grid)).ravel()
+    assert np.max(np.abs(got - U @ q)) < 1e-13
+
+
+def test_converges_to_matrix_exponential_order4(oracle):
+    """q(s=1) -> expm(Laplacian_spectral - diag w) 1 on 4^3, error falling ~16x per doubling of Ns."""
+    grid, cell = (4, 4, 4), (3.0, 4.0, 5.0)
+    M = 64
+    w = inputs.random_complex_field(grid, 3, scale=1.0, mean=0.5)
+    F = _dense_F(grid)
+    lap = (np.conj(F).T / M) @ np.diag(-_dense_k2(grid, cell)) @ F
+    exact = scipy.linalg.expm(lap - np.diag(w.ravel())) @ np.ones(M)
+    errs = []
+    for Ns in (16, 32, 64, 128, 256):
+        o = oracle.Oracle(grid, cell, Ns, "external")
+        o.set_fields(w)
+        o.propagate()
+        errs.append(np.max(np.abs(o.get_slice(0, Ns).ravel() - exact)))
+    ratios = [errs[i] / errs[i + 1] for i in range(4)]
+    assert errs[-1] < 1e-8
+    assert all(12.0 < r < 17.0 for r in ratios), (errs, ratios)     # rough field: 12.7, 14.1, 15, 15.5 -> 16
+    assert ratios[-1] > 15.0
+
+
+def test_order4_at_config1(oracle):
+    """Q(Ns) - Q(512) falls 16x per halving of ds on the config-1 field (PAPER.md:122 'globally fourth-order')."""
+    cfg = inputs.config1()
+    Qs = {}
+    for Ns in (8, 16, 32, 64, 512):
+        o = oracle.Oracle(cfg.grid, cfg.cell, Ns, "external")
+        o.set_fields(cfg.f0)
+        o.propagate()
+        Qs[Ns] = o.density_operators()[0]
+    errs = [abs(Qs[n] - Qs[512]) for n in (8, 16, 32, 64)]
+    ratios = [errs[i] / errs[i + 1] for i in range(3)]
+    assert all(12.0 < r < 18.0 for r in ratios), (errs, ratios)
+
+
+# ------------------------------------------------------------------ invariants ------------------
+@pytest.mark.parametrize("model", ["external", "diblock"])
+def test_qqdag_invariant_and_normalisation(oracle, model):
+    """(1/M) sum_x q_j q+_{Ns-j} = Q for every j (bilinear product, reading A-9); mean phi_A = fA, mean phi = 1."""
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=(4, 8, 16), Ns=20, fA=0.4)
+        o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "diblock", fA=cfg.fA, chiN=cfg.chiN)
+        o.set_fields(cfg.f0, cfg.f1)
+    else:
+        cfg = inputs.config1(grid=(8, 8, 8), Ns=16)
+        o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "external")
+        o.set_fields(cfg.f0)
+    o.propagate()
+    Q, pa, pb = o.density_operators()
+    for j in range(cfg.Ns + 1):
+        Qj = np.mean(o.get_slice(0, j) * o.get_slice(1, cfg.Ns - j))
+        assert abs(Qj - Q) < 1e-13 * abs(Q), j
+    assert abs(np.mean(o.get_slice(1, cfg.Ns)) - Q) < 1e-13 * abs(Q)            # Q[q+] = Q[q]
+    if model == "diblock":
+        assert abs(np.mean(pa) - cfg.fA) < 1e-12 and abs(np.mean(pa + pb) - 1.0) < 1e-12
+    else:
+        assert abs(np.mean(pa) - 1.0) < 1e-12
+
+
+# ------------------------------------------------------------------ Debye response --------------
+def _gD(x):
+    return 2.0 * (np.exp(-x) + x - 1.0) / x ** 2
+
+
+@pytest.mark.parametrize("n", [(1, 0, 0), (0, 1, 1), (2, 1, 0)])
+def test_debye_response_homopolymer(oracle, n):
+    """phi - 1 = -eps g_D(k^2) cos(k.x) for w = eps cos(k.x)   (north_star g_D)."""
+    grid, cell, Ns, eps = (16, 16, 16), (4.0, 4.0, 4.0), 64, 1e-4
+    X = np.meshgrid(*[np.arange(g) * (L / g) for g, L in zip(grid, cell)], indexing="ij")
+    th = 2 * np.pi * sum(n[d] * X[d] / cell[d] for d in range(3))
+    o = oracle.Oracle(grid, cell, Ns, "external")
+    o.set_fields((eps * np.cos(th)).astype(np.complex128))
+    o.propagate()
+    _, phi, _ = o.density_operators()
+    coef = 2.0 * np.mean((phi.real - 1.0) * np.cos(th))
+    k2 = sum((2 * np.pi * n[d] / cell[d]) ** 2 for d in range(3))
+    assert abs(coef / (-eps * _gD(k2)) - 1.0) < 2e-6
+
+
+def test_debye_response_diblock_blocks(oracle):
+    """Block-resolved response: phi_A - fA = -eps (g_AA + g_AB) cos, phi_A + phi_B - 1 = -eps g_D cos
+    for wA = wB = eps cos (textbook diblock Debye functions; pins the jA split and per-block Simpson)."""
+    grid, cell, Ns, fA, eps = (16, 1, 1), (4.0, 1.0, 1.0), 60, 0.3, 1e-4
+    x = np.arange(16) * (4.0 / 16)
+    th = (2 * np.pi * x / 4.0).reshape(grid)
+    o = oracle.Oracle(grid, cell, Ns, "diblock", fA=fA, chiN=10.0)
+    o.set_fields((eps * np.cos(th)).astype(np.complex128), np.zeros(grid, np.complex128))
+    o.propagate()
+    _, pa, pb = o.density_operators()
+    k2 = (2 * np.pi / 4.0) ** 2
+    gAA = 2.0 * (np.exp(-fA * k2) + fA * k2 - 1.0) / k2 ** 2
+    gAB = (1 - np.exp(-fA * k2)) * (1 - np.exp(-(1 - fA) * k2)) / k2 ** 2
+    cA = 2.0 * np.mean((pa.real - fA) * np.cos(th))
+    cT = 2.0 * np.mean((pa.real + pb.real - 1.0) * np.cos(th))
+    assert abs(cA / (-eps * (gAA + gAB)) - 1.0) < 2e-6
+    assert abs(cT / (-eps * _gD(k2)) - 1.0) < 2e-6
+    assert abs(oracle.debye(k2) - _gD(k2)) < 1e-15 and abs(oracle.debye(0.0) - 1.0) < 1e-15
+    from decimal import Decimal, getcontext
+    getcontext().prec = 60
+    for xs in ("0.00005", "0.009", "0.011", "0.5"):                                  # both branches vs 60-digit arithmetic
+        xd = Decimal(xs)
+        ref = 2 * ((-xd).exp() + xd - 1) / (xd * xd)
+        assert abs(oracle.debye(float(xs)) - float(ref)) < 1e-11
+
+
+# ------------------------------------------------------------------ saddles and field updates ---
+def test_diblock_homogeneous_saddle(oracle):
+    """W- = chiN(2fA-1)/2, any uniform W+: both forces vanish, H/CV = -chiN(1-2fA)^2/4."""
+    grid, Ns, fA, chiN = (4, 4, 4), 20, 0.3, 16.0
+    wm, wp = chiN * (2 * fA - 1) / 2, 0.37
+    o = oracle.Oracle(grid, (4.0,) * 3, Ns, "diblock", fA=fA, chiN=chiN)
+    o.set_fields(np.full(grid, wp, np.complex128), np.full(grid, wm, np.complex128))
+    H, resid = o.scft_step(5.0, 5.0, seidel=1)
+    assert abs(H - (-chiN * (1 - 2 * fA) ** 2 / 4)) < 1e-13
+    assert resid[0] < 1e-13 and resid[1] < 1e-13
+    a, b = o.get_fields()
+    assert np.max(np.abs(a - wp)) < 1e-12 and np.max(np.abs(b - wm)) < 1e-12
+
+
+@pytest.mark.parametrize("seidel", [0, 1])
+def test_scft_relaxes_to_mean_field_solution(oracle, seidel):
+    """1-D lamellar: residuals of the mean-field equations fall and H drops below the homogeneous value."""
+    grid, cell, Ns, fA, chiN = (32, 1, 1), (4.0, 1.0, 1.0), 40, 0.5, 20.0
+    x = np.arange(32) * (4.0 / 32)
+    wm = (2.0 * np.cos(2 * np.pi * x / 4.0)).reshape(grid).astype(np.complex128)
+    o = oracle.Oracle(grid, cell, Ns, "diblock", fA=fA, chiN=chiN)
+    o.set_fields(np.zeros(grid, np.complex128), wm)
+    res = []
+    for _ in range(80):
+        H, r = o.scft_step(5.0, 5.0, seidel=seidel)
+        res.append(max(r))
+    assert res[-1] < 1e-3 and res[-1] < 1e-2 * res[0]
+    assert H.real < -chiN * (1 - 2 * fA) ** 2 / 4 - 0.1 and abs(H.imag) < 1e-12
+    a, b = o.get_fields()
+    assert np.max(np.abs(a.imag)) < 1e-12 and np.max(np.abs(b.imag)) < 1e-12      # Wick-rotated fields stay real
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_edwards_noise_free_relaxation_reaches_saddle(oracle, scheme):
+    """Omega* = -iC/B, Q = exp(-C/B), mu = ln C + C/B, Pi = C + C^2/(2B)   (Eq. 2 as printed, reading A-13/A-14)."""
+    grid, Ns, B, Cc = (8, 8, 8), 8, 2.0, 3.0
+    rng = np.random.default_rng(5)
+    om = -1j * Cc / B + 0.05 * rng.normal(size=grid)
+    o = oracle.Oracle(grid, (4.0,) * 3, Ns, "edwards", B=B, Cc=Cc, noise_scale=0.0)
+    o.set_fields(om.astype(np.complex128))
+    for it in range(200):
+        o.cl_step(0.2, scheme, 1, it)
+    f, _ = o.get_fields()
+    assert np.max(np.abs(f - (-1j * Cc / B))) < 1e-9
+    o.propagate()
+    Q, _, _ = o.density_operators()
+    H, mu, Pi = o.operators()
+    assert abs(Q - np.exp(-Cc / B)) < 1e-9
+    assert abs(mu - (np.log(Cc) + Cc / B)) < 1e-9
+    assert abs(Pi - (Cc + Cc ** 2 / (2 * B))) < 1e-8
+
+
+def test_pressure_kernel_matches_volume_derivative_of_lnQ(oracle):
+    """-(2/3V) K = d ln Q / dV at fixed lattice fields (reading A-14; the only pin Pi has: 'parity unpinned')."""
+    cfg = inputs.config1(grid=(8, 8, 8), Ns=64)
+    V = float(np.prod(cfg.cell))
+
+    def lnQ(scale):
+        cell = tuple(L * scale ** (1 / 3) for L in cfg.cell)
+        o = oracle.Oracle(cfg.grid, cell, cfg.Ns, "external")
+        o.set_fields(cfg.f0)
+        o.propagate()
+        return np.log(o.density_operators()[0]), o
+
+    d = 1e-4
+    fd = (lnQ(1 + d)[0] - lnQ(1 - d)[0]) / (2 * d * V)
+    _, o = lnQ(1.0)
+    _, _, Pi = o.operators()                     # model 0: Pi = -(2/3) K
+    assert abs(Pi / V - fd) < 5e-3 * abs(fd)
+
+
+# ------------------------------------------------------------------ Philox / noise --------------
+def test_philox_known_answers(oracle):
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox4x32_10_kat.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        assert oracle.philox4x32_10(v[0:4], v[4:6]) == tuple(v[6:10])
+
+
+def test_normal_moments_and_noise_amplitude(oracle):
+    n = 200000
+    z = np.array([oracle.normal(99, 3, 1, i) for i in range(n)])
+    assert abs(z.mean()) < 4 / np.sqrt(n)
+    assert abs(z.var() - 1.0) < 4 * np.sqrt(2.0 / n)
+    assert abs(np.mean(z ** 4) - 3.0) < 4 * np.sqrt(96.0 / n)
+    assert oracle.normal(99, 3, 1, 5) != oracle.normal(99, 3, 0, 5) != oracle.normal(99, 4, 0, 5)
+    # Var eta = 2 lambda dt / dV: one Edwards CL step from a force-free state of B=0, C->0
+    grid, cell, dt = (8, 8, 8), (2.0, 2.0, 2.0), 0.01
+    o = oracle.Oracle(grid, cell, 4, "edwards", B=0.0, Cc=1e-300, lambda_plus=1.0)
+    o.set_fields(np.zeros(grid, np.complex128))
+    o.cl_step(dt, 0, 7, 0)
+    f, _ = o.get_fields()
+    dV = 8.0 / 512
+    assert np.max(np.abs(f.imag)) < 1e-200
+    assert abs(f.real.var() / (2 * dt / dV) - 1.0) < 4 * np.sqrt(2.0 / 512)
+    assert f.real.ravel()[5] == pytest.approx(np.sqrt(2 * dt / dV) * oracle.normal(7, 0, 0, 5), rel=1e-15)
+
+
+def test_cl_step_diblock_euler_maruyama_signs(oracle):
+    """Zero-noise EM step equals W+ + dt C (phiA+phiB-1), W- - dt C (2W-/chiN + phiB - phiA)."""
+    cfg = inputs.small_diblock(grid=(4, 4, 8), Ns=8, fA=0.5)
+    kw = dict(fA=cfg.fA, chiN=cfg.chiN, Cc=cfg.C)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "diblock", noise_scale=0.0, **kw)
+    o.set_fields(cfg.f0, cfg.f1)
+    o.propagate()
+    _, pa, pb = o.density_operators()
+    o.cl_step(0.01, 0, 1, 0)
+    a, b = o.get_fields()
+    assert np.max(np.abs(a - (cfg.f0 + 0.01 * cfg.C * (pa + pb - 1)))) < 1e-14
+    assert np.max(np.abs(b - (cfg.f1 - 0.01 * cfg.C * (2 * cfg.f1 / cfg.chiN + pb - pa)))) < 1e-14
+    # with noise: W+ gets i*eta, W- gets eta, independent streams (reading A-15)
+    o2 = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "diblock", **kw)
+    o2.set_fields(cfg.f0, cfg.f1)
+    o2.cl_step(0.01, 0, 42, 3)
+    a2, b2 = o2.get_fields()
+    M = int(np.prod(cfg.grid))
+    amp = np.sqrt(2 * 0.01 / (np.prod(cfg.cell) / M))
+    ep = np.array([oracle.normal(42, 3, 0, i) for i in range(M)]).reshape(cfg.grid)
+    em = np.array([oracle.normal(42, 3, 1, i) for i in range(M)]).reshape(cfg.grid)
+    assert np.max(np.abs((a2 - a) - 1j * amp * ep)) < 1e-13
+    assert np.max(np.abs((b2 - b) - amp * em)) < 1e-13
+
+
+def test_fp32_oracle_tracks_fp64(oracle):
+    cfg = inputs.config1(grid=(8, 8, 8), Ns=16)
+    Qs = []
+    for prec in ("f64", "f32"):
+        o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "external", precision=prec)
+        o.set_fields(cfg.f0)
+        o.propagate()
+        Qs.append(o.density_operators()[0])
+    assert abs(Qs[1] - Qs[0]) < 2e-5 * abs(Qs[0])
+
+
+def test_create_rejects_bad_arguments(oracle):
+    with pytest.raises(ValueError):
+        oracle.Oracle((4, 4, 4), (1.0,) * 3, 10, "diblock", fA=0.33)     # fA*Ns not an integer (reading A-4)
+    with pytest.raises(ValueError):
+        oracle.Oracle((4, 4, 4), (1.0,) * 3, 10, "diblock", fA=0.5)      # odd block (Simpson, reading A-5)
+    with pytest.raises(ValueError):
+        oracle.Oracle((4, 4, 4), (1.0,) * 3, 7, "external")
