@@ -1,0 +1,115 @@
+/* fts.h — C ABI of fts-b200: the hot path of polymer field-theoretic simulation on one NVIDIA B200.
+ *
+ * Method: Delaney & Fredrickson, "Polymer Field-Theory Simulations on Graphics Processing Units",
+ * arXiv 1204.5434 (text: PAPER.md, cited as PAPER.md:<line>).  The library solves the modified diffusion
+ * equation (Eq. 5) for the chain propagators q and q+ with the 4th-order Richardson-extrapolated
+ * pseudo-spectral step (Eq. 12), evaluates the single-chain partition function Q (PAPER.md:65
+ * Eq. 4) and the segment volume fractions phi_A, phi_B (Eq. 8), and advances the fields by one
+ * SCFT relaxation step or one complex-Langevin step (PAPER.md:102 Eq. 9, :112-118 Eq. 10-11).
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback and no cuFFT.
+ *
+ * Units and conventions: lengths in Rg, contour s in [0,1], ds = 1/Ns; the diffusion
+ * factor is exp(-k^2 ds).  Grids: shape (Nx,Ny,Nz), layout [ix][iy][iz] with z contiguous, interleaved
+ * (re,im); FTS_F64 = complex128, FTS_F32 = complex64.  Every grid dimension must be a power of two in
+ * [8, 256] (FTS_EUNSUPPORTED otherwise; the paper benchmarks power-of-two grids).
+ *
+ * Stored fields:  FTS_MODEL_EXTERNAL  f0 = w                       (one species in a given complex field)
+ *                 FTS_MODEL_EDWARDS   f0 = Omega                   (chain feels i*Omega; Eq. 2)
+ *                 FTS_MODEL_DIBLOCK   f0 = W+ = i*omega_+, f1 = W- = omega_-;  w_A = W+ - W-, w_B = W+ + W-
+ *                                                                  (Eq. 3)
+ *
+ * Ownership: every *_dev pointer and the workspace are DEVICE memory allocated by the caller; the library
+ * never allocates or frees device memory and keeps the workspace until fts_destroy.  Host outputs
+ * (double[2] = re, im) are fp64 in both precisions.  `stream` is a cudaStream_t passed as void*.
+ * All work is enqueued on `stream`; calls that return host scalars synchronise that stream.
+ *
+ * Errors: status codes only (no exceptions, no aborts); text of the last error from fts_last_error().
+ * Determinism: same inputs and same (seed, step) give bit-identical outputs run to run (fixed-order
+ * reductions, counter-based noise).
+ */
+#ifndef FTS_H
+#define FTS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fts_ctx fts_ctx;
+
+typedef enum {
+    FTS_OK = 0,
+    FTS_EINVAL = 1,        /* NULL pointer, Ns < 2, fA*Ns not an integer (1e-9), odd Simpson block, cell <= 0      */
+    FTS_ESTATE = 2,        /* call order: fields not set, density before propagate, slice not retained           */
+    FTS_EWORKSPACE = 3,    /* workspace smaller than fts_workspace_bytes, or not 256-byte aligned                   */
+    FTS_ECUDA = 4,         /* a CUDA call failed; text in fts_last_error                                          */
+    FTS_ENONFINITE = 5,    /* Q is NaN/Inf (diverged CL run)                                                       */
+    FTS_EUNSUPPORTED = 6   /* grid dimension not a power of two in [8,256]; model/step combination not defined    */
+} fts_status;
+
+typedef enum { FTS_F64 = 0, FTS_F32 = 1 } fts_precision;
+
+typedef enum { FTS_MODEL_EXTERNAL = 0, FTS_MODEL_EDWARDS = 1, FTS_MODEL_DIBLOCK = 2 } fts_model;
+
+typedef struct {
+    int    model;                       /* fts_model                                                              */
+    double fA, chiN, B, C;              /* block fraction, Flory parameter, excluded volume, chain density        */
+    double lambda_plus, lambda_minus;   /* mobilities of Eq. 9 (Edwards uses lambda_plus); 0 is read as 1        */
+    double noise_scale;                 /* multiplies eta in fts_cl_step: 1 = physical, 0 = deterministic         */
+    int    store_both;                  /* reserved: this version always keeps every q and q+ slice in HBM        */
+} fts_params;
+
+/* Bytes of device workspace fts_create needs: fields, Boltzmann factors, the contour-slice store
+ * ((Ns+1) slices per propagator; PAPER.md:183 memory analysis), scratch, tables. */
+fts_status fts_workspace_bytes(const int grid[3], int Ns, const fts_params* params, fts_precision prec, size_t* bytes);
+
+/* Builds the k-tables exp(-k_d^2 ds), exp(-k_d^2 ds/2) (once per simulation), the FFT
+ * twiddles and the Simpson weights, and lays out the workspace.  cell = box lengths in Rg. */
+fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts_params* params, fts_precision prec,
+                      void* workspace_dev, size_t workspace_bytes, fts_ctx** out);
+fts_status fts_destroy(fts_ctx* ctx);
+
+/* Copy fields into / out of the context (device to device).  f1_dev is NULL for one-field models. */
+fts_status fts_set_fields(fts_ctx* ctx, const void* f0_dev, const void* f1_dev, void* stream);
+fts_status fts_get_fields(fts_ctx* ctx, void* f0_dev, void* f1_dev, void* stream);
+
+/* PAPER.md:143 Boltzmann factors, then Ns RQM4 steps (Eq. 12) of q and, batched with it, q+ (diblock);
+ * every slice is written to the HBM store; Q = mean_x q(x,1) (Eq. 4) is left on the device.  Asynchronous. */
+fts_status fts_propagate(fts_ctx* ctx, void* stream);
+/* March only the first nsteps contour steps (truncated parity at 256^3); Q is then mean_x q_nsteps. */
+fts_status fts_propagate_steps(fts_ctx* ctx, int nsteps, void* stream);
+
+/* phi_A (and phi_B) = (ds/Q) sum_j c_j q_j q+_{Ns-j}, composite Simpson per block (Eq. 8; plain bilinear
+ * product).  Writes phi to caller memory, returns Q; synchronises `stream`.  phiB_dev NULL for one species. */
+fts_status fts_density_operators(fts_ctx* ctx, void* phiA_dev, void* phiB_dev, double Q_out[2], void* stream);
+
+/* Copy slice j of q (which = 0) or q+ (which = 1; q+ is indexed from the far chain end) to out_dev. */
+fts_status fts_get_slice(fts_ctx* ctx, int which, int j, void* out_dev, void* stream);
+
+/* One SCFT iteration for the diblock melt (PAPER.md:84 forces; Eq. 11 at zero noise): W+ ascends with the
+ * Debye-linearised response implicit, W- descends with its explicit linear term implicit.  seidel = 1
+ * re-solves the propagators between the two updates (2 solves per iteration), seidel = 0 uses one solve.
+ * H_out = H/(CV) of the fields at entry; resid_out = max|F+|, max|F-|.  Synchronises `stream`. */
+fts_status fts_scft_step(fts_ctx* ctx, double dt_plus, double dt_minus, int seidel, double H_out[2], double resid_out[2], void* stream);
+
+/* One complex-Langevin step (Eq. 9).  scheme 0 = Euler-Maruyama in real space; scheme 1 = the first-order
+ * semi-implicit update of Eq. 10-11.  Noise: Philox4x32-10 keyed by `seed`, counter (site, step, field id),
+ * Box-Muller, variance 2 lambda dt / dV, generated inside the update kernel.  Asynchronous. */
+fts_status fts_cl_step(fts_ctx* ctx, double dt, int scheme, uint64_t seed, uint64_t step, void* stream);
+
+/* Operators of the current fields; needs a completed fts_propagate.  H: Eq. 2 (Edwards, extensive) or
+ * Eq. 3 / (CV) (diblock); mu = ln C - ln Q; Pi: volume derivative of ln Z at fixed lattice fields (derived in
+ * DESIGN.md, not printed in the paper: secondary output).  Any pointer may be NULL.  Synchronises `stream`. */
+fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], void* stream);
+
+/* Raw Philox4x32-10 block and the standard normal fts_cl_step draws for (seed, step, field, site), evaluated
+ * ON THE DEVICE for n consecutive sites starting at site0; out_dev receives n doubles.  For tests. */
+fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream);
+
+const char* fts_last_error(const fts_ctx* ctx);
+const char* fts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,525 @@
+// fts_api.cu — host side of the C-ABI library declared in include/fts.h: context, workspace layout,
+// host-built tables (S1), the launch schedule of one RQM4 contour step (S3-S5), Q (S7), densities (S6),
+// field updates (S8-S9) and operators (S10).  No device allocation happens here: everything lives in
+// the caller's workspace.  No CPU fallback: every arithmetic step of the path is a kernel in fts_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fts.h"
+#include "fts_kernels.cuh"
+
+namespace fts {
+
+static const long double kPiL = 3.14159265358979323846264338327950288L;
+
+struct DimTables { void* tab[2]; void* tw; double* k2; };
+
+struct Ctx {
+    int g[3]; double L[3]; int Ns; fts_params P; fts_precision prec;
+    size_t M; int nprop, nspecies, jA; size_t esz;
+    char* ws; size_t ws_bytes;
+    // workspace carve-up
+    DimTables dim[3];
+    double *cA, *cB, *scal, *kacc; double2* partial;
+    void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2];
+    bool have_fields, have_prop; int marched;
+    std::string err;
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Layout {          // the single place that decides where things live in the workspace
+    size_t off_tab[3][2], off_tw[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial;
+    size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], total;
+};
+static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
+    Layout Lo; size_t o = 0;
+    const size_t M = (size_t)g[0] * g[1] * g[2], field = align_up(M * esz);
+    const int nprop = model == FTS_MODEL_DIBLOCK ? 2 : 1;
+    for (int d = 0; d < 3; ++d) {
+        for (int h = 0; h < 2; ++h) { Lo.off_tab[d][h] = o; o += align_up((size_t)g[d] * esz / 2); }
+        Lo.off_tw[d] = o; o += align_up((size_t)g[d] * esz);
+        Lo.off_k2[d] = o; o += align_up((size_t)g[d] * sizeof(double));
+    }
+    Lo.off_cA = o; o += align_up((size_t)(Ns + 1) * sizeof(double));
+    Lo.off_cB = o; o += align_up((size_t)(Ns + 1) * sizeof(double));
+    Lo.off_scal = o; o += align_up(64 * sizeof(double));
+    Lo.off_kacc = o; o += align_up((size_t)(Ns + 1) * 2 * sizeof(double));
+    Lo.off_partial = o; o += align_up(1024 * sizeof(double2));
+    for (int i = 0; i < 2; ++i) { Lo.off_f[i] = o; o += field; }
+    for (int i = 0; i < 2; ++i) { Lo.off_e4[i] = o; o += field; }
+    for (int i = 0; i < 2; ++i) { Lo.off_F[i] = o; o += (i < nprop) ? field : 0; }
+    for (int i = 0; i < 2; ++i) { Lo.off_H[i] = o; o += (i < nprop) ? field : 0; }
+    for (int i = 0; i < 2; ++i) { Lo.off_phi[i] = o; o += field; }
+    for (int i = 0; i < 2; ++i) { Lo.off_G[i] = o; o += field; }
+    for (int i = 0; i < 2; ++i) { Lo.off_q[i] = o; o += (i < nprop) ? align_up((size_t)(Ns + 1) * M * esz) : 0; }   // contour-slice store
+    Lo.total = o;
+    return Lo;
+}
+
+static bool pow2_ok(int n) { return n >= 8 && n <= 256 && (n & (n - 1)) == 0; }
+
+static fts_status validate(const int grid[3], const double* cell, int Ns, const fts_params* P, int prec) {
+    if (!grid || !P) return FTS_EINVAL;
+    if (prec != FTS_F64 && prec != FTS_F32) return FTS_EINVAL;
+    if (Ns < 2 || P->model < 0 || P->model > 2) return FTS_EINVAL;
+    for (int d = 0; d < 3; ++d) {
+        if (grid[d] < 1) return FTS_EINVAL;
+        if (cell && !(cell[d] > 0)) return FTS_EINVAL;
+    }
+    if (P->model == FTS_MODEL_DIBLOCK) {
+        const double x = P->fA * Ns; const long j = std::lround(x);
+        if (std::fabs(x - (double)j) > 1e-9 || j <= 0 || j >= Ns) return FTS_EINVAL;     // reading A-4
+        if ((j & 1) || ((Ns - j) & 1)) return FTS_EINVAL;                                  // reading A-5 (Simpson)
+        if (!(P->chiN > 0)) return FTS_EINVAL;
+    } else if (Ns & 1) return FTS_EINVAL;
+    for (int d = 0; d < 3; ++d) if (!pow2_ok(grid[d])) return FTS_EUNSUPPORTED;
+    return FTS_OK;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                           \
+            return FTS_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// pass launch: picks the instantiation for (precision, pencil length, strided or contiguous)
+// ------------------------------------------------------------------------------------------------
+template <class T, int N, int EPT, int TZ>
+static cudaError_t launch_pass_inst(const PassArgs& A, int njobs, cudaStream_t st) {
+    typedef PassCfg<T, N, EPT, TZ> Cfg;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid((A.ntiles + Cfg::GPB - 1) / Cfg::GPB, njobs);
+    pass_kernel<T, N, EPT, TZ><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    return cudaGetLastError();
+}
+template <class T, int TZ>
+static cudaError_t launch_pass_n(int N, const PassArgs& A, int njobs, cudaStream_t st) {
+    switch (N) {
+        case 8: return launch_pass_inst<T, 8, 8, TZ>(A, njobs, st);
+        case 16: return launch_pass_inst<T, 16, 16, TZ>(A, njobs, st);
+        case 32: return launch_pass_inst<T, 32, 8, TZ>(A, njobs, st);
+        case 64: return launch_pass_inst<T, 64, 8, TZ>(A, njobs, st);
+        case 128: return launch_pass_inst<T, 128, 16, TZ>(A, njobs, st);
+        case 256: return launch_pass_inst<T, 256, 16, TZ>(A, njobs, st);
+    }
+    return cudaErrorInvalidValue;
+}
+template <class T> constexpr int tz_of() { return 128 / (2 * (int)sizeof(T)); }   // 128-byte rows
+
+// dim: 0 = x, 1 = y (strided pencils, tiles of TZ consecutive z), 2 = z (contiguous pencils)
+template <class T>
+static cudaError_t launch_pass(const Ctx* c, int dim, PassArgs A, int njobs, cudaStream_t st) {
+    const int Nx = c->g[0], Ny = c->g[1], Nz = c->g[2];
+    A.tab[0] = c->dim[dim].tab[0]; A.tab[1] = c->dim[dim].tab[1]; A.tw = c->dim[dim].tw;
+    A.k2x = c->dim[0].k2; A.k2y = c->dim[1].k2; A.k2z = c->dim[2].k2; A.Nz = Nz;
+    A.invN = 1.0 / (double)c->g[dim];
+    if (dim == 2) {
+        A.pstride = 1; A.outer_stride = 0; A.tiles_inner = 1; A.ntiles = Nx * Ny;
+        return launch_pass_n<T, 0>(Nz, A, njobs, st);
+    }
+    constexpr int TZ = tz_of<T>();
+    const int tz = Nz < TZ ? 8 : TZ;                       // complex64 with Nz = 8: 64-byte rows
+    if (dim == 0) { A.pstride = Ny * Nz; A.outer_stride = 0; A.tiles_inner = Ny * Nz / tz; A.ntiles = Ny * Nz / tz; }
+    else { A.pstride = Nz; A.outer_stride = Ny * Nz; A.tiles_inner = Nz / tz; A.ntiles = Nx * Nz / tz; }
+    if (tz == TZ) return launch_pass_n<T, TZ>(c->g[dim], A, njobs, st);
+    return launch_pass_n<T, 8>(c->g[dim], A, njobs, st);
+}
+
+static Job mkjob(const void* in, void* out, int op, int pre = PRE_NONE, int tabA = 0, const void* e4 = nullptr, int second = 0, int tabB = 0,
+                 int post = POST_NONE, const void* aux = nullptr) {
+    Job j; j.in = in; j.out = out; j.e4 = e4; j.aux = aux; j.op = op; j.pre = pre; j.tabA = tabA; j.second = second; j.tabB = tabB; j.post = post;
+    return j;
+}
+
+static int ew_blocks(size_t M) { size_t b = (M + 255) / 256; return (int)(b < 148 * 16 ? b : 148 * 16); }
+
+template <class T, int OP>
+static cudaError_t reduce(const Ctx* c, const void* a, const void* b, double p, double scale, double* out_dev, cudaStream_t st) {
+    const int M = (int)c->M;
+    int nb = (M + RED_THREADS - 1) / RED_THREADS; if (nb > RED_BLOCKS) nb = RED_BLOCKS;
+    reduce_partial_kernel<T, OP><<<nb, RED_THREADS, 0, st>>>((const cplx<T>*)a, (const cplx<T>*)b, M, p, c->partial);
+    reduce_final_kernel<OP><<<1, 1024, 0, st>>>(c->partial, nb, scale, out_dev);
+    return cudaGetLastError();
+}
+
+// scalar slots in c->scal
+enum { S_Q = 0, S_H = 2, S_RP = 4, S_RM = 6, S_SQ = 8, S_Q0 = 10 };
+
+// ------------------------------------------------------------------------------------------------
+// S2-S7: the march.  Per contour step, five fused passes over the {q, q+} batch:
+//   X1: F = Dx[e2 q],  H = Dx'[e4 q]      Y1: F = Dy F, H = Dy' H      Z: F = e2 Dz F, H = Dz'[e2 Dz' H]
+//   Y2: H = Dy' H                          X2: q' = (4 e4 Dx' H - F)/3  -> slice store
+// (D = full-step factor exp(-k_d^2 ds), D' = half-step factor; the three 1-D factors commute.)
+// ------------------------------------------------------------------------------------------------
+template <class T>
+static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
+    const size_t M = c->M; const int Ns = c->Ns, np = c->nprop;
+    const double ds = 1.0 / Ns;
+    boltzmann_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)c->e4[0], (cplx<T>*)c->e4[1], (int)M, c->P.model, ds / 4);
+    for (int b = 0; b < np; ++b) fill_kernel<T><<<ew_blocks(M), 256, 0, st>>>((cplx<T>*)c->q[b], (int)M, (T)1, (T)0);   // q(x,0) = 1, q+(x,s=1) = 1
+    CK(cudaGetLastError());
+    for (int j = 0; j < nsteps; ++j) {
+        const void* e4b[2]; const cplx<T>* qin[2]; cplx<T>* qout[2];
+        for (int b = 0; b < np; ++b) {
+            int sp = 0;
+            if (c->nspecies == 2) sp = (b == 0) ? (j >= c->jA ? 1 : 0) : (j < Ns - c->jA ? 1 : 0);      // O5 / O6 species schedule
+            e4b[b] = c->e4[sp];
+            qin[b] = (const cplx<T>*)c->q[b] + (size_t)j * M;
+            qout[b] = (cplx<T>*)c->q[b] + (size_t)(j + 1) * M;
+        }
+        PassArgs A; std::memset(&A, 0, sizeof A);
+        int n = 0;
+        for (int b = 0; b < np; ++b) {
+            A.job[n++] = mkjob(qin[b], c->F[b], OP_D, PRE_E2, 0, e4b[b]);
+            A.job[n++] = mkjob(qin[b], c->H[b], OP_D, PRE_E4, 1, e4b[b]);
+        }
+        CK(launch_pass<T>(c, 0, A, n, st));
+        n = 0;
+        for (int b = 0; b < np; ++b) { A.job[n++] = mkjob(c->F[b], c->F[b], OP_D, PRE_NONE, 0); A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1); }
+        CK(launch_pass<T>(c, 1, A, n, st));
+        n = 0;
+        for (int b = 0; b < np; ++b) {
+            A.job[n++] = mkjob(c->F[b], c->F[b], OP_D, PRE_NONE, 0, e4b[b], 0, 0, POST_E2);
+            A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1, e4b[b], 1, 1);
+        }
+        CK(launch_pass<T>(c, 2, A, n, st));
+        n = 0;
+        for (int b = 0; b < np; ++b) A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1);
+        CK(launch_pass<T>(c, 1, A, n, st));
+        n = 0;
+        for (int b = 0; b < np; ++b) A.job[n++] = mkjob(c->H[b], qout[b], OP_D, PRE_NONE, 1, e4b[b], 0, 0, POST_COMBINE, c->F[b]);
+        CK(launch_pass<T>(c, 0, A, n, st));
+    }
+    // S7 (Eq. 4): Q = (1/M) sum_x q_Ns(x), fixed-order tree
+    CK((reduce<T, RED_SUM>(c, (const cplx<T>*)c->q[0] + (size_t)nsteps * M, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st)));
+    c->marched = nsteps; c->have_prop = true;
+    return FTS_OK;
+}
+
+template <class T>
+static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
+    const cplx<T>* q = (const cplx<T>*)c->q[0];
+    const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];              // homopolymer: q+ == q
+    density_kernel<T><<<(unsigned)((c->M + 255) / 256), 256, 0, st>>>(q, qd, c->M, c->Ns, c->cA, c->cB, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA,
+                                                                       c->nspecies == 2 ? (cplx<T>*)phiB : nullptr);
+    CK(cudaGetLastError());
+    return FTS_OK;
+}
+
+// F^-1{ filt(k^2) F{g} } in place: z and y forward passes, x pass with the 3-D multiplier, y and z inverse passes
+template <class T>
+static fts_status filter3d_t(Ctx* c, void* g, Filt f, cudaStream_t st) {
+    PassArgs A; std::memset(&A, 0, sizeof A);
+    A.job[0] = mkjob(g, g, OP_FWD);
+    CK(launch_pass<T>(c, 2, A, 1, st));
+    CK(launch_pass<T>(c, 1, A, 1, st));
+    A.job[0] = mkjob(g, g, OP_FILT); A.filt = f;
+    CK(launch_pass<T>(c, 0, A, 1, st));
+    A.job[0] = mkjob(g, g, OP_INV);
+    CK(launch_pass<T>(c, 1, A, 1, st));
+    CK(launch_pass<T>(c, 2, A, 1, st));
+    return FTS_OK;
+}
+
+static fts_status read_scalars(Ctx* c, double* host, int n, cudaStream_t st) {
+    CK(cudaMemcpyAsync(host, c->scal, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return FTS_OK;
+}
+
+template <class T>
+static fts_status scft_step_t(Ctx* c, double dtp, double dtm, int seidel, double* Ho, double* ro, cudaStream_t st) {
+    const int M = (int)c->M; const int nb = ew_blocks(c->M);
+    fts_status rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
+    rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
+    CK(cudaMemcpyAsync(c->scal + S_Q0, c->scal + S_Q, 2 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CK((reduce<T, RED_DIBLOCK_H>(c, c->f0, c->f1, 1.0 / c->P.chiN, 1.0 / (double)M, c->scal + S_H, st)));
+    force_plus_kernel<T><<<nb, 256, 0, st>>>((const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M);
+    CK((reduce<T, RED_MAXABS>(c, c->G[0], nullptr, 0.0, 1.0, c->scal + S_RP, st)));
+    Filt f; f.type = FILT_RATIONAL; f.a = dtp; f.b = 0.0; f.c = dtp;                 // dt+/(1 + dt+ g_D(k^2))   (Eq. 11, reading A-10)
+    rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
+    add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+    if (seidel) {
+        rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
+        rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
+    }
+    scft_minus_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f1, (const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M, (T)(2.0 / c->P.chiN),
+                                             (T)(dtm / (1.0 + dtm * 2.0 / c->P.chiN)));
+    CK((reduce<T, RED_MAXABS>(c, c->G[0], nullptr, 0.0, 1.0, c->scal + S_RM, st)));
+    double h[12];
+    rc = read_scalars(c, h, 12, st); if (rc) return rc;
+    c->have_prop = false;
+    const double qx = h[S_Q0], qy = h[S_Q0 + 1];
+    if (!std::isfinite(qx) || !std::isfinite(qy)) return FTS_ENONFINITE;
+    if (Ho) { Ho[0] = h[S_H] - 0.5 * std::log(qx * qx + qy * qy); Ho[1] = h[S_H + 1] - std::atan2(qy, qx); }     // H/(CV) = mean[...] - ln Q
+    if (ro) { ro[0] = h[S_RP]; ro[1] = h[S_RM]; }
+    return FTS_OK;
+}
+
+template <class T>
+static fts_status cl_step_t(Ctx* c, double dt, int scheme, uint64_t seed, uint64_t step, cudaStream_t st) {
+    const int M = (int)c->M; const int nb = ew_blocks(c->M);
+    fts_status rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
+    rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
+    const double dV = c->L[0] * c->L[1] * c->L[2] / (double)c->M;
+    const double lp = c->P.lambda_plus, lm = c->P.lambda_minus, ns = c->P.noise_scale;
+    if (c->P.model == FTS_MODEL_EDWARDS) {
+        const double amp = ns * std::sqrt(2.0 * lp * dt / dV);
+        cl_edwards_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->phi[0], (cplx<T>*)c->G[0], M, lp * dt, c->P.B, c->P.C, amp, seed, step, scheme == 0);
+        CK(cudaGetLastError());
+        if (scheme == 1) {
+            Filt f; f.type = FILT_RATIONAL; f.a = 1.0; f.b = lp * dt * c->P.B; f.c = lp * dt * c->P.C;
+            rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
+            add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+        }
+    } else {
+        const double ap = ns * std::sqrt(2.0 * lp * dt / dV), am = ns * std::sqrt(2.0 * lm * dt / dV);
+        const double dm = scheme == 1 ? 1.0 / (1.0 + lm * dt * 2.0 * c->P.C / c->P.chiN) : 1.0;
+        cl_diblock_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (cplx<T>*)c->f1, (const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M, lp * dt * c->P.C,
+                                                 lm * dt * c->P.C, 2.0 / c->P.chiN, ap, am, dm, seed, step, scheme == 0);
+        CK(cudaGetLastError());
+        if (scheme == 1) {
+            Filt f; f.type = FILT_RATIONAL; f.a = 1.0; f.b = 0.0; f.c = lp * dt * c->P.C;
+            rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
+            add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+        }
+    }
+    CK(cudaGetLastError());
+    c->have_prop = false;
+    return FTS_OK;
+}
+
+// S10 operators (PAPER.md:50 Eq. 2, :54 Eq. 3, :183; readings A-14, A-17)
+template <class T>
+static fts_status operators_t(Ctx* c, double* Ho, double* muo, double* Pio, cudaStream_t st) {
+    const size_t M = c->M; const int Ns = c->Ns;
+    const cplx<T>* q = (const cplx<T>*)c->q[0];
+    const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];
+    fts_status rc;
+    if (Pio) {                                             // K_j = (1/M) sum_x q+_{Ns-j} Laplacian(q_j)
+        Filt f; f.type = FILT_NEGK2; f.a = 1.0; f.b = f.c = 0.0;
+        for (int j = 0; j <= Ns; ++j) {
+            CK(cudaMemcpyAsync(c->G[0], q + (size_t)j * M, M * sizeof(cplx<T>), cudaMemcpyDeviceToDevice, st));
+            rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
+            CK((reduce<T, RED_PROD>(c, c->G[0], qd + (size_t)(Ns - j) * M, 0.0, 1.0 / (double)M, c->kacc + 2 * j, st)));
+        }
+    }
+    if (c->P.model == FTS_MODEL_EDWARDS) CK((reduce<T, RED_SUMSQ>(c, c->f0, nullptr, 0.0, 1.0, c->scal + S_SQ, st)));
+    if (c->P.model == FTS_MODEL_DIBLOCK) CK((reduce<T, RED_DIBLOCK_H>(c, c->f0, c->f1, 1.0 / c->P.chiN, 1.0 / (double)M, c->scal + S_H, st)));
+    std::vector<double> kh(2 * (Ns + 1), 0.0);
+    if (Pio) CK(cudaMemcpyAsync(kh.data(), c->kacc, kh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+    double h[12];
+    rc = read_scalars(c, h, 12, st); if (rc) return rc;
+    const double qx = h[S_Q], qy = h[S_Q + 1];
+    if (!std::isfinite(qx) || !std::isfinite(qy)) return FTS_ENONFINITE;
+    const double lnQ[2] = {0.5 * std::log(qx * qx + qy * qy), std::atan2(qy, qx)};
+    double K[2] = {0, 0};
+    if (Pio) {
+        std::vector<double> wA(Ns + 1), wB(Ns + 1);
+        CK(cudaMemcpy(wA.data(), c->cA, (Ns + 1) * sizeof(double), cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(wB.data(), c->cB, (Ns + 1) * sizeof(double), cudaMemcpyDeviceToHost));
+        double sx = 0, sy = 0;
+        for (int j = 0; j <= Ns; ++j) { const double w = wA[j] + wB[j]; sx += w * kh[2 * j]; sy += w * kh[2 * j + 1]; }
+        const double ds = 1.0 / Ns, den = qx * qx + qy * qy;
+        K[0] = ds * (sx * qx + sy * qy) / den; K[1] = ds * (sy * qx - sx * qy) / den;
+    }
+    const double V = c->L[0] * c->L[1] * c->L[2], dV = V / (double)M, Cc = c->P.C, B = c->P.B;
+    double H[2], mu[2], Pi[2];
+    if (c->P.model == FTS_MODEL_EDWARDS) {
+        H[0] = 0.5 * B * dV * h[S_SQ] - Cc * V * lnQ[0]; H[1] = 0.5 * B * dV * h[S_SQ + 1] - Cc * V * lnQ[1];
+        mu[0] = std::log(Cc) - lnQ[0]; mu[1] = -lnQ[1];
+        Pi[0] = Cc - 0.5 * B * dV * h[S_SQ] / V - (2.0 * Cc / 3.0) * K[0]; Pi[1] = -0.5 * B * dV * h[S_SQ + 1] / V - (2.0 * Cc / 3.0) * K[1];
+    } else if (c->P.model == FTS_MODEL_DIBLOCK) {
+        H[0] = h[S_H] - lnQ[0]; H[1] = h[S_H + 1] - lnQ[1];
+        mu[0] = std::log(Cc > 0 ? Cc : 1.0) - lnQ[0]; mu[1] = -lnQ[1];
+        Pi[0] = Cc - (2.0 * Cc / 3.0) * K[0]; Pi[1] = -(2.0 * Cc / 3.0) * K[1];
+    } else {
+        H[0] = -lnQ[0]; H[1] = -lnQ[1]; mu[0] = -lnQ[0]; mu[1] = -lnQ[1];
+        Pi[0] = -(2.0 / 3.0) * K[0]; Pi[1] = -(2.0 / 3.0) * K[1];
+    }
+    if (Ho) { Ho[0] = H[0]; Ho[1] = H[1]; }
+    if (muo) { muo[0] = mu[0]; muo[1] = mu[1]; }
+    if (Pio) { Pio[0] = Pi[0]; Pio[1] = Pi[1]; }
+    return FTS_OK;
+}
+
+static double simpson_weight(int j, int a, int b) {     // composite Simpson 1/3 on [a,b], 0 outside (reading A-5)
+    if (j < a || j > b) return 0.0;
+    if (j == a || j == b) return 1.0 / 3.0;
+    return ((j - a) & 1) ? 4.0 / 3.0 : 2.0 / 3.0;
+}
+
+// S1: everything that is computed once per simulation
+template <class T>
+static fts_status build_tables(Ctx* c) {
+    const double ds = 1.0 / c->Ns;
+    for (int d = 0; d < 3; ++d) {
+        const int N = c->g[d];
+        std::vector<T> t0(N), t1(N); std::vector<cplx<T>> tw(N); std::vector<double> k2(N);
+        for (int i = 0; i < N; ++i) {
+            const int n = (i <= N / 2) ? i : i - N;
+            const long double k = 2.0L * kPiL * (long double)n / (long double)c->L[d];
+            k2[i] = (double)(k * k);
+            t0[i] = (T)((double)std::exp(-(k * k) * (long double)ds) / (double)N);             // inverse-FFT 1/N folded in
+            t1[i] = (T)((double)std::exp(-(k * k) * (long double)ds * 0.5L) / (double)N);
+            const long double a = -2.0L * kPiL * (long double)i / (long double)N;
+            tw[i] = mk<T>((T)std::cos(a), (T)std::sin(a));
+        }
+        CK(cudaMemcpy(c->dim[d].tab[0], t0.data(), N * sizeof(T), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(c->dim[d].tab[1], t1.data(), N * sizeof(T), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(c->dim[d].tw, tw.data(), N * sizeof(cplx<T>), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(c->dim[d].k2, k2.data(), N * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    std::vector<double> wA(c->Ns + 1), wB(c->Ns + 1);
+    for (int j = 0; j <= c->Ns; ++j) { wA[j] = simpson_weight(j, 0, c->jA); wB[j] = c->nspecies == 2 ? simpson_weight(j, c->jA, c->Ns) : 0.0; }
+    CK(cudaMemcpy(c->cA, wA.data(), wA.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->cB, wB.data(), wB.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CK(cudaMemset(c->scal, 0, 64 * sizeof(double)));
+    return FTS_OK;
+}
+
+}  // namespace fts
+
+using namespace fts;
+struct fts_ctx : fts::Ctx {};
+
+#define DISPATCH(expr_f64, expr_f32) (c->prec == FTS_F64 ? (expr_f64) : (expr_f32))
+
+extern "C" {
+
+const char* fts_version(void) { return "fts-b200 0.1 (sm_100a)"; }
+const char* fts_last_error(const fts_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+fts_status fts_workspace_bytes(const int grid[3], int Ns, const fts_params* P, fts_precision prec, size_t* bytes) {
+    if (!bytes) return FTS_EINVAL;
+    fts_status rc = validate(grid, nullptr, Ns, P, prec); if (rc) return rc;
+    *bytes = make_layout(grid, Ns, P->model, prec == FTS_F64 ? 16 : 8).total;
+    return FTS_OK;
+}
+
+fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts_params* P, fts_precision prec, void* ws, size_t ws_bytes, fts_ctx** out) {
+    if (!cell || !out || !ws) return FTS_EINVAL;
+    fts_status rc = validate(grid, cell, Ns, P, prec); if (rc) return rc;
+    const size_t esz = prec == FTS_F64 ? 16 : 8;
+    const Layout Lo = make_layout(grid, Ns, P->model, esz);
+    if (ws_bytes < Lo.total || ((uintptr_t)ws & 255)) return FTS_EWORKSPACE;
+    fts_ctx* c = new (std::nothrow) fts_ctx;
+    if (!c) return FTS_EINVAL;
+    for (int d = 0; d < 3; ++d) { c->g[d] = grid[d]; c->L[d] = cell[d]; }
+    c->Ns = Ns; c->P = *P; c->prec = prec; c->esz = esz;
+    if (!(c->P.lambda_plus > 0)) c->P.lambda_plus = 1.0;
+    if (!(c->P.lambda_minus > 0)) c->P.lambda_minus = 1.0;
+    c->M = (size_t)grid[0] * grid[1] * grid[2];
+    c->nprop = c->nspecies = (P->model == FTS_MODEL_DIBLOCK) ? 2 : 1;
+    c->jA = (P->model == FTS_MODEL_DIBLOCK) ? (int)std::lround(P->fA * Ns) : Ns;
+    c->ws = (char*)ws; c->ws_bytes = ws_bytes;
+    for (int d = 0; d < 3; ++d) {
+        c->dim[d].tab[0] = c->ws + Lo.off_tab[d][0]; c->dim[d].tab[1] = c->ws + Lo.off_tab[d][1];
+        c->dim[d].tw = c->ws + Lo.off_tw[d]; c->dim[d].k2 = (double*)(c->ws + Lo.off_k2[d]);
+    }
+    c->cA = (double*)(c->ws + Lo.off_cA); c->cB = (double*)(c->ws + Lo.off_cB);
+    c->scal = (double*)(c->ws + Lo.off_scal); c->kacc = (double*)(c->ws + Lo.off_kacc); c->partial = (double2*)(c->ws + Lo.off_partial);
+    c->f0 = c->ws + Lo.off_f[0]; c->f1 = c->ws + Lo.off_f[1];
+    for (int i = 0; i < 2; ++i) {
+        c->e4[i] = c->ws + Lo.off_e4[i]; c->F[i] = c->ws + Lo.off_F[i]; c->H[i] = c->ws + Lo.off_H[i];
+        c->q[i] = c->ws + Lo.off_q[i]; c->phi[i] = c->ws + Lo.off_phi[i]; c->G[i] = c->ws + Lo.off_G[i];
+    }
+    c->have_fields = c->have_prop = false; c->marched = 0;
+    rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
+    if (rc) { delete c; return rc; }
+    *out = c;
+    return FTS_OK;
+}
+
+fts_status fts_destroy(fts_ctx* c) { delete c; return FTS_OK; }
+
+fts_status fts_set_fields(fts_ctx* c, const void* f0, const void* f1, void* stream) {
+    if (!c || !f0 || (c->P.model == FTS_MODEL_DIBLOCK && !f1)) return FTS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(c->f0, f0, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
+    if (c->P.model == FTS_MODEL_DIBLOCK) CK(cudaMemcpyAsync(c->f1, f1, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
+    c->have_fields = true; c->have_prop = false;
+    return FTS_OK;
+}
+fts_status fts_get_fields(fts_ctx* c, void* f0, void* f1, void* stream) {
+    if (!c) return FTS_EINVAL;
+    if (!c->have_fields) return FTS_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (f0) CK(cudaMemcpyAsync(f0, c->f0, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
+    if (f1 && c->P.model == FTS_MODEL_DIBLOCK) CK(cudaMemcpyAsync(f1, c->f1, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
+    return FTS_OK;
+}
+
+fts_status fts_propagate_steps(fts_ctx* c, int nsteps, void* stream) {
+    if (!c || nsteps < 0 || nsteps > c->Ns) return FTS_EINVAL;
+    if (!c->have_fields) return FTS_ESTATE;
+    return DISPATCH(propagate_t<double>(c, nsteps, (cudaStream_t)stream), propagate_t<float>(c, nsteps, (cudaStream_t)stream));
+}
+fts_status fts_propagate(fts_ctx* c, void* stream) { return c ? fts_propagate_steps(c, c->Ns, stream) : FTS_EINVAL; }
+
+fts_status fts_density_operators(fts_ctx* c, void* phiA, void* phiB, double Q_out[2], void* stream) {
+    if (!c || !phiA || (c->nspecies == 2 && !phiB)) return FTS_EINVAL;
+    if (!c->have_prop || c->marched != c->Ns) return FTS_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    fts_status rc = DISPATCH(density_t<double>(c, phiA, phiB, st), density_t<float>(c, phiA, phiB, st));
+    if (rc) return rc;
+    double h[2];
+    rc = read_scalars(c, h, 2, st); if (rc) return rc;
+    if (Q_out) { Q_out[0] = h[0]; Q_out[1] = h[1]; }
+    if (!std::isfinite(h[0]) || !std::isfinite(h[1])) return FTS_ENONFINITE;
+    return FTS_OK;
+}
+
+fts_status fts_get_slice(fts_ctx* c, int which, int j, void* out, void* stream) {
+    if (!c || !out || which < 0 || which > 1 || j < 0 || j > c->Ns) return FTS_EINVAL;
+    if (!c->have_prop || j > c->marched) return FTS_ESTATE;
+    const char* base = (const char*)c->q[which == 1 ? c->nprop - 1 : 0];
+    CK(cudaMemcpyAsync(out, base + (size_t)j * c->M * c->esz, c->M * c->esz, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return FTS_OK;
+}
+
+fts_status fts_scft_step(fts_ctx* c, double dtp, double dtm, int seidel, double H[2], double resid[2], void* stream) {
+    if (!c || !(dtp > 0) || !(dtm > 0)) return FTS_EINVAL;
+    if (c->P.model != FTS_MODEL_DIBLOCK) return FTS_EUNSUPPORTED;
+    if (!c->have_fields) return FTS_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    return DISPATCH(scft_step_t<double>(c, dtp, dtm, seidel, H, resid, st), scft_step_t<float>(c, dtp, dtm, seidel, H, resid, st));
+}
+
+fts_status fts_cl_step(fts_ctx* c, double dt, int scheme, uint64_t seed, uint64_t step, void* stream) {
+    if (!c || !(dt > 0) || scheme < 0 || scheme > 1) return FTS_EINVAL;
+    if (c->P.model == FTS_MODEL_EXTERNAL) return FTS_EUNSUPPORTED;
+    if (!c->have_fields) return FTS_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    return DISPATCH(cl_step_t<double>(c, dt, scheme, seed, step, st), cl_step_t<float>(c, dt, scheme, seed, step, st));
+}
+
+fts_status fts_operators(fts_ctx* c, double H[2], double mu[2], double Pi[2], void* stream) {
+    if (!c) return FTS_EINVAL;
+    if (!c->have_prop || c->marched != c->Ns) return FTS_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    return DISPATCH(operators_t<double>(c, H, mu, Pi, st), operators_t<float>(c, H, mu, Pi, st));
+}
+
+fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream) {
+    if (!out_dev) return FTS_EINVAL;
+    if (n == 0) return FTS_OK;
+    normals_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, field_id, site0, n, out_dev);
+    return cudaGetLastError() == cudaSuccess ? FTS_OK : FTS_ECUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,386 @@
+// fts_kernels.cuh — sm_100a kernels of the fts-b200 hot path.
+//
+// pass_kernel       one launch = one fused 1-D pass over up to four fields ("jobs"): load pencils into registers,
+//                   optional real-space Boltzmann multiply, [FFT -> spectral multiply -> IFFT] along the pencil with
+//                   one shared-memory exchange per transform, optional second diffusion (the z-pass of the half
+//                   branch), optional epilogue (Boltzmann multiply or the Richardson combine of PAPER.md:124 Eq. 12).
+// boltzmann_kernel  exp(-w ds/4) per species.
+// reduce_kernel     deterministic two-level sums / max (Q of Eq. 4, H of Eq. 2-3, residuals).
+// density_kernel    Simpson contour sums of q_j q+_{Ns-j} (Eq. 8).
+// update kernels    forces of PAPER.md:84, Euler-Maruyama / semi-implicit updates of Eq. 9-11, Philox noise.
+#ifndef FTS_KERNELS_CUH
+#define FTS_KERNELS_CUH
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fts_pencil.h"
+
+namespace fts {
+
+enum { OP_D = 0, OP_FWD = 1, OP_INV = 2, OP_FILT = 3 };
+enum { PRE_NONE = 0, PRE_E4 = 1, PRE_E2 = 2 };
+enum { POST_NONE = 0, POST_E2 = 1, POST_COMBINE = 2 };
+enum { FILT_RATIONAL = 0, FILT_NEGK2 = 1 };
+
+struct Job {                  // block-uniform description of one field's trip through a pass
+    const void* in;
+    void* out;
+    const void* e4;           // exp(-w ds/4) of the species this step uses (e2 = e4*e4)
+    const void* aux;          // full-step branch, for POST_COMBINE
+    int op, pre, tabA, second, tabB, post;
+};
+
+struct Filt { int type; double a, b, c; };   // RATIONAL: a / (1 + b + c*g_D(k^2));  NEGK2: -a*k^2
+
+struct PassArgs {
+    Job job[4];
+    const void* tab[2];       // real tables of this dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
+    const void* tw;           // exp(-2 pi i m / N), m = 0..N-1
+    int pstride;              // element stride along the pencil
+    int outer_stride;         // strided passes: tile -> base offset = (tile / tiles_inner)*outer_stride + (tile % tiles_inner)*TZ
+    int tiles_inner;
+    int ntiles;               // strided: number of [N][TZ] tiles;  contiguous: number of pencils
+    Filt filt;                // OP_FILT only (x pass): 3-D multiplier built from the three k_d^2 tables
+    const double* k2x; const double* k2y; const double* k2z;
+    int Nz;
+    double invN;
+};
+
+template <class T, int N, int EPT, int TZ>
+struct PassCfg {
+    typedef PencilShape<N, EPT> S;
+    static constexpr bool CONTIG = (TZ == 0);
+    static constexpr int TARGET = 128;
+    static constexpr int GROUP = CONTIG ? S::TPP : TZ * S::TPP;                 // threads that exchange among themselves
+    static constexpr int GPB = (TARGET / GROUP) > 0 ? (TARGET / GROUP) : 1;     // tiles (strided) or pencils (contiguous) per CTA
+    static constexpr int THREADS = GROUP * GPB;
+    static constexpr int PS = CONTIG ? contig_ps<T, N, EPT>() : 1;
+    static constexpr int XELEMS = S::ONE ? 0 : (CONTIG ? GPB * PS : GPB * N * TZ);   // one exchange buffer, in complex elements
+    typedef typename std::conditional<CONTIG, XchgLayout<PS, S::R2 + 1, 1>, XchgLayout<1, S::R2 * (TZ ? TZ : 1), (TZ ? TZ : 1)>>::type L;
+    static constexpr size_t SMEM = (size_t)N * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T) + 2 * (size_t)XELEMS * sizeof(cplx<T>);
+};
+
+__device__ __forceinline__ double debye_dev(double x) {          // g_D(x) = 2(e^-x + x - 1)/x^2
+    if (x < 1e-2) return 1.0 - x * (1.0 / 3.0) + x * x * (1.0 / 12.0) - x * x * x * (1.0 / 60.0) + x * x * x * x * (1.0 / 360.0);
+    return 2.0 * (exp(-x) + x - 1.0) / (x * x);
+}
+__device__ __forceinline__ double filt_eval(const Filt& f, double k2) {
+    return f.type == FILT_NEGK2 ? -f.a * k2 : f.a / (1.0 + f.b + f.c * debye_dev(k2));
+}
+
+template <class T, int N, int EPT, int TZ>
+__global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(const PassArgs A) {
+    typedef PassCfg<T, N, EPT, TZ> Cfg;
+    typedef Pencil<T, N, EPT> P;
+    typedef typename Cfg::S S;
+    typedef typename Cfg::L L;
+    typedef cplx<T> C;
+    constexpr int TPP = S::TPP;
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* s_tw = reinterpret_cast<C*>(smem_raw);
+    T* s_tab = reinterpret_cast<T*>(s_tw + N);
+    C* s_x0 = reinterpret_cast<C*>(s_tab + 2 * N);
+    C* s_x1 = s_x0 + Cfg::XELEMS;
+
+    const int tid = threadIdx.x;
+    for (int i = tid; i < N; i += Cfg::THREADS) {
+        s_tw[i] = static_cast<const C*>(A.tw)[i];
+        s_tab[i] = static_cast<const T*>(A.tab[0])[i];
+        s_tab[N + i] = static_cast<const T*>(A.tab[1])[i];
+    }
+    __syncthreads();
+
+    const Job J = A.job[blockIdx.y];
+    int t, p, base, ps;
+    bool active;
+    if constexpr (Cfg::CONTIG) {
+        t = tid % TPP;
+        p = tid / TPP;
+        const int pencil = blockIdx.x * Cfg::GPB + p;
+        active = pencil < A.ntiles;
+        base = pencil * N;
+        ps = 1;
+    } else {
+        const int zz = tid % TZ, tb = tid / (TZ * TPP);
+        t = (tid / TZ) % TPP;
+        const int tile = blockIdx.x * Cfg::GPB + tb;
+        active = tile < A.ntiles;
+        base = (tile / A.tiles_inner) * A.outer_stride + (tile % A.tiles_inner) * TZ + zz;
+        ps = A.pstride;
+        p = zz;
+        s_x0 += tb * (N * TZ);
+        s_x1 += tb * (N * TZ);
+    }
+
+    const C* in = static_cast<const C*>(J.in);
+    const C* e4 = static_cast<const C*>(J.e4);
+    C v[EPT];
+#pragma unroll
+    for (int r = 0; r < EPT; ++r) v[r] = active ? in[base + (t + TPP * r) * ps] : mk<T>(0, 0);
+    if (J.pre != PRE_NONE) {
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) {
+            C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
+            if (J.pre == PRE_E2) e = e * e;
+            v[r] = v[r] * e;
+        }
+    }
+
+    auto forward = [&]() {
+        P::fwd_a(v, t, s_tw);
+        if constexpr (!S::ONE) {
+            P::template xchg_store_a<L>(v, t, s_x0, p);
+            __syncthreads();
+            P::template xchg_load_b<L>(v, t, s_x0, p);
+        }
+        P::fwd_b(v);
+    };
+    auto inverse = [&]() {
+        P::inv_b(v);
+        if constexpr (!S::ONE) {
+            P::template xchg_store_b<L>(v, t, s_x1, p);
+            __syncthreads();
+            P::template xchg_load_a<L>(v, t, s_x1, p);
+        }
+        P::inv_a(v, t, s_tw);
+    };
+
+    if (J.op == OP_D) {
+        forward();
+        const T* tab = s_tab + J.tabA * N;
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) v[r] = v[r] * tab[t + TPP * r];
+        inverse();
+        if (J.second) {       // z pass of the half branch: D_z^{1/2} e2 D_z^{1/2}
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) {
+                C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
+                v[r] = v[r] * (e * e);
+            }
+            forward();
+            const T* tabb = s_tab + J.tabB * N;
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) v[r] = v[r] * tabb[t + TPP * r];
+            inverse();
+        }
+    } else if (J.op == OP_FWD) {
+        forward();
+    } else if (J.op == OP_INV) {
+        const T s = (T)A.invN;
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) v[r] = v[r] * s;
+        inverse();
+    } else {                  // OP_FILT: forward, 3-D multiplier, inverse (x pass of the field-update transforms)
+        forward();
+        const int c = base % A.pstride;               // offset inside the yz plane = iy*Nz + iz
+        const double kyz = A.k2y[c / A.Nz] + A.k2z[c % A.Nz];
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) v[r] = v[r] * (T)(filt_eval(A.filt, A.k2x[t + TPP * r] + kyz) * A.invN);
+        inverse();
+    }
+
+    C* out = static_cast<C*>(J.out);
+    if (J.post == POST_E2) {
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) {
+            C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
+            v[r] = v[r] * (e * e);
+        }
+    } else if (J.post == POST_COMBINE) {   // q' = (4 e4 half - full)/3   (Eq. 12)
+        const C* aux = static_cast<const C*>(J.aux);
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) {
+            const int idx = base + (t + TPP * r) * ps;
+            C e = active ? e4[idx] : mk<T>(0, 0);
+            C f = active ? aux[idx] : mk<T>(0, 0);
+            C h = v[r] * e;
+            v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
+        }
+    }
+    if (active) {
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) out[base + (t + TPP * r) * ps] = v[r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// elementwise kernels
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void fill_kernel(cplx<T>* a, int M, T re, T im) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) a[i] = mk<T>(re, im);
+}
+
+__device__ __forceinline__ cplx<double> cexp_d(cplx<double> z) {
+    double s, c;
+    sincos(z.y, &s, &c);
+    const double m = exp(z.x);
+    return mk<double>(m * c, m * s);
+}
+
+// S2: species field from the stored fields, then e4 = exp(-w ds/4); evaluated in fp64, rounded to T.
+// model 0: w = f0; 1: w = i*f0; 2: wA = f0 - f1, wB = f0 + f1.
+template <class T>
+__global__ void boltzmann_kernel(const cplx<T>* f0, const cplx<T>* f1, cplx<T>* e4A, cplx<T>* e4B, int M, int model, double ds4) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        cplx<double> a = mk<double>((double)f0[i].x, (double)f0[i].y);
+        if (model == 1) a = mk<double>(-a.y, a.x);
+        if (model == 2) {
+            cplx<double> b = mk<double>((double)f1[i].x, (double)f1[i].y);
+            cplx<double> eb = cexp_d(mk<double>(-(a.x + b.x) * ds4, -(a.y + b.y) * ds4));
+            e4B[i] = mk<T>((T)eb.x, (T)eb.y);
+            a = a - b;
+        }
+        cplx<double> ea = cexp_d(mk<double>(-a.x * ds4, -a.y * ds4));
+        e4A[i] = mk<T>((T)ea.x, (T)ea.y);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// deterministic reductions: fixed grid, fixed per-thread order, fixed shared-memory tree
+// ------------------------------------------------------------------------------------------------
+enum { RED_SUM = 0, RED_SUMSQ = 1, RED_PROD = 2, RED_DIBLOCK_H = 3, RED_MAXABS = 4 };
+constexpr int RED_BLOCKS = 592, RED_THREADS = 256;     // 4 CTAs per SM on 148 SMs
+
+template <class T, int OP>
+__device__ __forceinline__ double2 red_value(const cplx<T>* a, const cplx<T>* b, int i, double p) {
+    const double ax = (double)a[i].x, ay = (double)a[i].y;
+    if constexpr (OP == RED_SUM) return make_double2(ax, ay);
+    else if constexpr (OP == RED_SUMSQ) return make_double2(ax * ax - ay * ay, 2.0 * ax * ay);
+    else if constexpr (OP == RED_PROD) { const double bx = (double)b[i].x, by = (double)b[i].y; return make_double2(ax * bx - ay * by, ax * by + ay * bx); }
+    else if constexpr (OP == RED_DIBLOCK_H) {           // W-^2/chiN - W+ with a = W+, b = W-, p = 1/chiN   (Eq. 3)
+        const double bx = (double)b[i].x, by = (double)b[i].y;
+        return make_double2((bx * bx - by * by) * p - ax, 2.0 * bx * by * p - ay);
+    } else return make_double2(sqrt(ax * ax + ay * ay), 0.0);
+}
+template <int OP> __device__ __forceinline__ double2 red_comb(double2 u, double2 w) {
+    if constexpr (OP == RED_MAXABS) return make_double2(fmax(u.x, w.x), 0.0);
+    else return make_double2(u.x + w.x, u.y + w.y);
+}
+
+template <class T, int OP>
+__global__ void __launch_bounds__(RED_THREADS) reduce_partial_kernel(const cplx<T>* a, const cplx<T>* b, int M, double p, double2* partial) {
+    __shared__ double2 sm[RED_THREADS];
+    double2 acc = make_double2(0.0, 0.0);
+    for (int i = blockIdx.x * RED_THREADS + threadIdx.x; i < M; i += gridDim.x * RED_THREADS) acc = red_comb<OP>(acc, red_value<T, OP>(a, b, i, p));
+    sm[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = RED_THREADS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sm[threadIdx.x] = red_comb<OP>(sm[threadIdx.x], sm[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
+}
+template <int OP>
+__global__ void __launch_bounds__(1024) reduce_final_kernel(const double2* partial, int n, double scale, double* out) {
+    __shared__ double2 sm[1024];
+    sm[threadIdx.x] = threadIdx.x < n ? partial[threadIdx.x] : make_double2(0.0, 0.0);
+    __syncthreads();
+    for (int s = 512; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sm[threadIdx.x] = red_comb<OP>(sm[threadIdx.x], sm[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sm[0].x * scale; out[1] = sm[0].y * scale; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S6 density (Eq. 8): phi_A = (ds/Q) sum_j cA_j q_j q+_{Ns-j}, phi_B likewise; fp64 accumulators
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) density_kernel(const cplx<T>* q, const cplx<T>* qd, size_t M, int Ns, const double* cA, const double* cB,
+                                                      const double* Qdev, double ds, cplx<T>* phiA, cplx<T>* phiB) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    double ax = 0, ay = 0, bx = 0, by = 0;
+#pragma unroll 4
+    for (int j = 0; j <= Ns; ++j) {
+        const cplx<T> u = q[(size_t)j * M + i], w = qd[(size_t)(Ns - j) * M + i];
+        const double px = (double)u.x * (double)w.x - (double)u.y * (double)w.y, py = (double)u.x * (double)w.y + (double)u.y * (double)w.x;
+        const double wa = cA[j], wb = cB[j];
+        ax += wa * px; ay += wa * py;
+        bx += wb * px; by += wb * py;
+    }
+    const double qx = Qdev[0], qy = Qdev[1], den = ds / (qx * qx + qy * qy);     // multiply by ds * conj(Q)/|Q|^2
+    phiA[i] = mk<T>((T)((ax * qx + ay * qy) * den), (T)((ay * qx - ax * qy) * den));
+    if (phiB) phiB[i] = mk<T>((T)((bx * qx + by * qy) * den), (T)((by * qx - bx * qy) * den));
+}
+
+// ------------------------------------------------------------------------------------------------
+// S9 noise: Philox4x32-10 (Salmon et al., SC'11) + Box-Muller, one normal per (site, field, step)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t (&o)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+__device__ __forceinline__ double normal_dev(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site) {
+    uint32_t o[4];
+    philox4x32_10((uint32_t)site, (uint32_t)(site >> 32), (uint32_t)step, field_id ^ ((uint32_t)(step >> 32) << 8), (uint32_t)seed, (uint32_t)(seed >> 32), o);
+    const uint64_t m1 = ((uint64_t)o[0] << 21) | (o[1] >> 11), m2 = ((uint64_t)o[2] << 21) | (o[3] >> 11);
+    const double u1 = (double)(m1 + 1) * 0x1p-53, u2 = (double)(m2 + 1) * 0x1p-53;
+    return sqrt(-2.0 * log(u1)) * cos(2.0 * 3.14159265358979323846264338327950288 * u2);
+}
+__global__ void normals_kernel(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = normal_dev(seed, step, field_id, site0 + i);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S8 forces and field updates (PAPER.md:84; :102 Eq. 9; :112-118 Eq. 10-11; readings A-10, A-11, A-15)
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void force_plus_kernel(const cplx<T>* phiA, const cplx<T>* phiB, cplx<T>* g, int M) {      // F+ = phiA + phiB - 1
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x)
+        g[i] = mk<T>(phiA[i].x + phiB[i].x - (T)1, phiA[i].y + phiB[i].y);
+}
+template <class T>
+__global__ void add_kernel(cplx<T>* w, const cplx<T>* g, int M) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) w[i] = w[i] + g[i];
+}
+// F- = 2 W-/chiN + phiB - phiA (stored in g for the residual), W- -= coef * F-
+template <class T>
+__global__ void scft_minus_kernel(cplx<T>* wm, const cplx<T>* phiA, const cplx<T>* phiB, cplx<T>* g, int M, T two_over_chi, T coef) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        const cplx<T> w = wm[i];
+        const cplx<T> F = mk<T>(two_over_chi * w.x + phiB[i].x - phiA[i].x, two_over_chi * w.y + phiB[i].y - phiA[i].y);
+        g[i] = F;
+        wm[i] = mk<T>(w.x - coef * F.x, w.y - coef * F.y);
+    }
+}
+// diblock CL numerators: np = l+ dt C (phiA+phiB-1) + i eta+,  nm = (-l- dt C (2W-/chiN + phiB - phiA) + eta-) * dm.
+// direct = 1 (Euler-Maruyama, or after the filter): fields are advanced in place; direct = 0: np -> g0, nm applied to W-.
+template <class T>
+__global__ void cl_diblock_kernel(cplx<T>* wp, cplx<T>* wm, const cplx<T>* phiA, const cplx<T>* phiB, cplx<T>* g0, int M, double cp, double cm,
+                                  double two_over_chi, double ampp, double ampm, double dm, uint64_t seed, uint64_t step, int direct) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        const cplx<T> a = phiA[i], b = phiB[i], m = wm[i];
+        const T ep = (T)(ampp * normal_dev(seed, step, 0u, (uint64_t)i)), em = (T)(ampm * normal_dev(seed, step, 1u, (uint64_t)i));
+        const cplx<T> np = mk<T>((T)cp * (a.x + b.x - (T)1), (T)cp * (a.y + b.y) + ep);
+        const cplx<T> Fm = mk<T>((T)two_over_chi * m.x + b.x - a.x, (T)two_over_chi * m.y + b.y - a.y);
+        const cplx<T> nm = mk<T>((-(T)cm * Fm.x + em) * (T)dm, (-(T)cm * Fm.y) * (T)dm);
+        if (direct) wp[i] = wp[i] + np; else g0[i] = np;
+        wm[i] = m + nm;
+    }
+}
+// Edwards: num = -l dt (B Omega + i C phi) + eta
+template <class T>
+__global__ void cl_edwards_kernel(cplx<T>* om, const cplx<T>* phi, cplx<T>* g0, int M, double ldt, double B, double Cc, double amp, uint64_t seed, uint64_t step, int direct) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        const cplx<T> o = om[i], f = phi[i];
+        const cplx<T> F = mk<T>((T)B * o.x - (T)Cc * f.y, (T)B * o.y + (T)Cc * f.x);
+        const T eta = (T)(amp * normal_dev(seed, step, 0u, (uint64_t)i));
+        const cplx<T> num = mk<T>(-(T)ldt * F.x + eta, -(T)ldt * F.y);
+        if (direct) om[i] = o + num; else g0[i] = num;
+    }
+}
+
+}  // namespace fts
+#endif

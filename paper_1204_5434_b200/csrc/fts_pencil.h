@@ -1,0 +1,205 @@
+// fts_pencil.h — register-resident 1-D pencil transforms for the fused diffusion passes.
+//
+// A "pencil" is one line of N grid points along x, y or z.  TPP = N/EPT threads share a pencil, each
+// holding EPT complex values in registers.  The transform of length N = R1*R2 is two register-level
+// radix-R butterflies (R <= 16) with ONE shared-memory exchange between them; for N <= 16 a single
+// thread holds the whole pencil and no exchange is needed.  Used as forward -> multiply by a real table
+// -> inverse, which is the operator exp(ds * d^2/dx_d^2) of PAPER.md:124-127 (Eq. 12) along one dimension;
+// the 3-D operator is the product of the three 1-D ones because exp(-k^2 ds) factorises.
+//
+// Layout facts the kernels rely on (checked on the host by tests/test_host_pencil.py):
+//   * natural layout:  register r of thread t holds point  n = t + TPP*r
+//   * spectral layout: register r of thread t holds mode   k = t + TPP*r   (same map: tables need no permutation)
+//
+// Everything here is __host__ __device__ so the index arithmetic can be exercised on the CPU.
+#ifndef FTS_PENCIL_H
+#define FTS_PENCIL_H
+
+#if defined(__CUDACC__)
+#define FTS_HD __host__ __device__ __forceinline__
+#else
+#define FTS_HD inline
+#endif
+
+#include <type_traits>
+
+namespace fts {
+
+template <class T> struct alignas(2 * sizeof(T)) cplx { T x, y; };
+
+template <class T> FTS_HD cplx<T> mk(T a, T b) { cplx<T> r; r.x = a; r.y = b; return r; }
+template <class T> FTS_HD cplx<T> operator+(cplx<T> a, cplx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
+template <class T> FTS_HD cplx<T> operator-(cplx<T> a, cplx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
+template <class T> FTS_HD cplx<T> operator*(cplx<T> a, cplx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <class T> FTS_HD cplx<T> operator*(cplx<T> a, T s) { return mk<T>(a.x * s, a.y * s); }
+template <class T> FTS_HD cplx<T> conj(cplx<T> a) { return mk<T>(a.x, -a.y); }
+
+// cos(2 pi m / 16), m = 0..4, correctly rounded literals; everything else by symmetry.
+FTS_HD constexpr double cos16_q(int m) {
+    return m == 0 ? 1.0 : m == 1 ? 0.92387953251128675613 : m == 2 ? 0.70710678118654752440 : m == 3 ? 0.38268343236508977173 : 0.0;
+}
+FTS_HD constexpr double cos16(int m) {          // any integer m
+    m = ((m % 16) + 16) % 16;
+    return m <= 4 ? cos16_q(m) : m <= 8 ? -cos16_q(8 - m) : m <= 12 ? -cos16_q(m - 8) : cos16_q(16 - m);
+}
+FTS_HD constexpr double sin16(int m) { return cos16(m - 4); }
+
+// multiply by exp(DIR * 2 pi i * NUM / 16) with the trivial cases folded at compile time
+template <int NUM, int DIR, class T>
+FTS_HD cplx<T> mul_w16(cplx<T> a) {
+    constexpr int m = (((NUM * (DIR < 0 ? -1 : 1)) % 16) + 16) % 16;
+    if constexpr (m == 0) return a;
+    else if constexpr (m == 4) return mk<T>(-a.y, a.x);      // * i
+    else if constexpr (m == 8) return mk<T>(-a.x, -a.y);
+    else if constexpr (m == 12) return mk<T>(a.y, -a.x);     // * -i
+    else if constexpr (m % 4 == 2) {                         // (+-1 +- i)/sqrt(2): 2 adds + 2 muls
+        constexpr T h = (T)0.70710678118654752440;
+        constexpr T sc = (T)(cos16(m) > 0 ? 1 : -1), ss = (T)(sin16(m) > 0 ? 1 : -1);
+        return mk<T>((sc * a.x - ss * a.y) * h, (ss * a.x + sc * a.y) * h);
+    } else {
+        constexpr T c = (T)cos16(m), s = (T)sin16(m);
+        return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
+    }
+}
+
+template <int B, int E, class F>
+FTS_HD void static_for(F&& f) {
+    if constexpr (B < E) {
+        f(std::integral_constant<int, B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
+constexpr int bitrev(int i, int bits) { int r = 0; for (int b = 0; b < bits; ++b) r |= ((i >> b) & 1) << (bits - 1 - b); return r; }
+constexpr int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+// In-register DFT of R = 2,4,8,16 points held at v[OFF + S*i], i = 0..R-1.  DIR = -1 forward (e^{-i...}),
+// +1 inverse (unnormalised).  Decimation in frequency, radix-2 stages, natural order in and out
+// (the bit reversal is a compile-time register renaming).
+template <int R, int S, int OFF, int DIR, class T, int NV>
+FTS_HD void dft_reg(cplx<T> (&v)[NV]) {
+    if constexpr (R > 1) {
+        static_for<0, ilog2(R)>([&](auto st) {
+            constexpr int half = R >> (decltype(st)::value + 1);
+            static_for<0, R / 2>([&](auto bi) {
+                constexpr int b = decltype(bi)::value;
+                constexpr int base = (b / half) * 2 * half, i = b % half;
+                constexpr int p0 = OFF + S * (base + i), p1 = OFF + S * (base + i + half);
+                cplx<T> a = v[p0], c = v[p1];
+                v[p0] = a + c;
+                v[p1] = mul_w16<i * (8 / half), DIR>(a - c);
+            });
+        });
+        cplx<T> tmp[R];
+        static_for<0, R>([&](auto ii) { constexpr int i = decltype(ii)::value; tmp[i] = v[OFF + S * bitrev(i, ilog2(R))]; });
+        static_for<0, R>([&](auto ii) { constexpr int i = decltype(ii)::value; v[OFF + S * i] = tmp[i]; });
+    }
+}
+
+// Factorisation of a pencil of N points over threads holding EPT values each.
+template <int N, int EPT>
+struct PencilShape {
+    static constexpr int TPP = N / EPT;                 // threads per pencil
+    static constexpr bool ONE = (TPP == 1);             // whole pencil in one thread
+    static constexpr int R1 = ONE ? N : EPT;            // first-stage radix (stride R2 in n)
+    static constexpr int R2 = ONE ? 1 : N / R1;         // second-stage radix
+    static constexpr int G1 = EPT / R1;                 // first-stage butterflies per thread
+    static constexpr int G2 = ONE ? 1 : EPT / R2;       // second-stage butterflies per thread
+    static_assert(N % EPT == 0 && R1 * R2 == N && R1 <= 16 && R2 <= 16 && R2 <= EPT, "unsupported pencil shape");
+    static_assert(ONE || (TPP * G1 == R2 && TPP * G2 == R1), "inconsistent pencil shape");
+};
+
+// Shared-memory addressing of the exchange buffer.  An element of the intermediate Y[n2][k1] of pencil
+// `p` (p = pencil slot inside the CTA) lives at  p*PS + k1*ROW + n2*ES  (in complex elements).
+//   strided passes (x, y): PS = 1, ES = TZ, ROW = R2*TZ   -> lanes = consecutive pencils, conflict-free
+//   contiguous pass (z):   ES = 1, ROW = R2+1, PS = padded pencil stride chosen by the caller
+template <int PS_, int ROW_, int ES_> struct XchgLayout { static constexpr int PS = PS_, ROW = ROW_, ES = ES_; };
+
+// Padded pencil stride (in complex elements) of the contiguous-pass exchange buffer: rows of R2+1 (odd), and
+// PS = TPP (mod lanes-per-phase) so that the pencils sharing one shared-memory phase hit disjoint banks.
+template <class T, int N, int EPT>
+constexpr int contig_ps() {
+    typedef PencilShape<N, EPT> S;
+    constexpr int lpp = 128 / (2 * (int)sizeof(T));       // lanes per shared-memory phase: 8 (complex128) or 16 (complex64)
+    int ps = S::R1 * (S::R2 + 1);
+    if (S::TPP < lpp) while (ps % lpp != S::TPP % lpp) ++ps;
+    return ps;
+}
+
+template <class T, int N, int EPT>
+struct Pencil {
+    typedef PencilShape<N, EPT> S;
+    typedef cplx<T> C;
+
+    // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.  tw[m] = exp(-2 pi i m / N).
+    template <class TW>
+    static FTS_HD void fwd_a(C (&v)[EPT], int t, const TW* tw) {
+        static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, -1>(v); });
+        if constexpr (!S::ONE) {
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                if constexpr (k1 > 0) {
+                    TW w = tw[(t + S::TPP * g) * k1];
+                    v[r] = v[r] * mk<T>((T)w.x, (T)w.y);
+                }
+            });
+        }
+    }
+    // exchange A -> B: after store + barrier + load, register g' + G2*n2 of thread t holds Y[n2][k1 = t + TPP*g'].
+    template <class L>
+    static FTS_HD void xchg_store_a(const C (&v)[EPT], int t, C* sm, int p) {
+        if constexpr (!S::ONE)
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                sm[p * L::PS + k1 * L::ROW + (t + S::TPP * g) * L::ES] = v[r];
+            });
+    }
+    template <class L>
+    static FTS_HD void xchg_load_b(C (&v)[EPT], int t, const C* sm, int p) {
+        if constexpr (!S::ONE)
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g2 = r % S::G2, n2 = r / S::G2;
+                v[r] = sm[p * L::PS + (t + S::TPP * g2) * L::ROW + n2 * L::ES];
+            });
+    }
+    // forward part B: radix-R2 butterflies.  Afterwards register r of thread t holds mode k = t + TPP*r.
+    static FTS_HD void fwd_b(C (&v)[EPT]) {
+        if constexpr (!S::ONE) static_for<0, S::G2>([&](auto g) { dft_reg<S::R2, S::G2, decltype(g)::value, -1>(v); });
+    }
+    // inverse = the mirror image: part B (radix-R2), exchange B -> A, part A (conjugate twiddle, radix-R1).
+    static FTS_HD void inv_b(C (&v)[EPT]) {
+        if constexpr (!S::ONE) static_for<0, S::G2>([&](auto g) { dft_reg<S::R2, S::G2, decltype(g)::value, +1>(v); });
+    }
+    template <class L>
+    static FTS_HD void xchg_store_b(const C (&v)[EPT], int t, C* sm, int p) {
+        if constexpr (!S::ONE)
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g2 = r % S::G2, n2 = r / S::G2;
+                sm[p * L::PS + (t + S::TPP * g2) * L::ROW + n2 * L::ES] = v[r];
+            });
+    }
+    template <class L>
+    static FTS_HD void xchg_load_a(C (&v)[EPT], int t, const C* sm, int p) {
+        if constexpr (!S::ONE)
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                v[r] = sm[p * L::PS + k1 * L::ROW + (t + S::TPP * g) * L::ES];
+            });
+    }
+    template <class TW>
+    static FTS_HD void inv_a(C (&v)[EPT], int t, const TW* tw) {
+        if constexpr (!S::ONE) {
+            static_for<0, EPT>([&](auto rr) {
+                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                if constexpr (k1 > 0) {
+                    TW w = tw[(t + S::TPP * g) * k1];
+                    v[r] = v[r] * mk<T>((T)w.x, -(T)w.y);
+                }
+            });
+        }
+        static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, +1>(v); });
+    }
+};
+
+}  // namespace fts
+#endif

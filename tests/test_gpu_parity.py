@@ -1,0 +1,202 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element by element, same seeded inputs.
+
+Tolerances (BASELINE.json north_star): fp64 1e-11 relative on Q, 1e-9 max-abs on phi and q(r,1);
+fp32 2e-4 relative; CL trajectories with identical Philox noise 1e-8 after 10 steps (fp64).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1204_5434_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_1204_5434_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _dev(a, dtype=torch.complex128):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0").to(dtype).contiguous()
+
+
+def _kw(cfg):
+    return dict(fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
+
+
+def _pair(B, oracle, cfg, precision="f64", **extra):
+    kw = _kw(cfg); kw.update(extra)
+    dt = torch.complex128 if precision == "f64" else torch.complex64
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **kw)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **kw)    # the fp64 oracle judges both precisions
+    f1 = None if cfg.f1 is None else _dev(cfg.f1, dt)
+    g.set_fields(_dev(cfg.f0, dt), f1)
+    o.set_fields(cfg.f0, cfg.f1)
+    return g, o
+
+
+def _cmp_solve(g, o, tolQ, tolphi, two):
+    g.propagate(); o.propagate()
+    Qg, pa, pb = g.density_operators()
+    Qo, oa, ob = o.density_operators()
+    assert abs(Qg - Qo) <= tolQ * abs(Qo), (Qg, Qo)
+    assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tolphi
+    if two:
+        assert np.max(np.abs(pb.cpu().numpy() - ob)) <= tolphi
+    return Qg
+
+
+def test_config1_fp64(B, oracle):
+    cfg = inputs.config1()
+    g, o = _pair(B, oracle, cfg)
+    _cmp_solve(g, o, 1e-11, 1e-9, False)
+    for j in (1, 2, 33, cfg.Ns):
+        assert np.max(np.abs(g.get_slice(0, j).cpu().numpy() - o.get_slice(0, j))) < 1e-9, j
+
+
+def test_config1_fp32(B, oracle):
+    cfg = inputs.config1()
+    g, o = _pair(B, oracle, cfg, precision="f32")
+    g.propagate(); o.propagate()
+    Qg, pa, _ = g.density_operators()
+    Qo, oa, _ = o.density_operators()
+    assert abs(Qg - Qo) < 2e-4 * abs(Qo)
+    assert np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 * np.max(np.abs(oa))
+
+
+@pytest.mark.parametrize("grid", [(8, 16, 32), (32, 8, 16), (16, 64, 8), (64, 32, 16)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_ragged_diblock_complex_fields(B, oracle, grid, precision):
+    """Anisotropic grids: every pencil length 8..64 appears along every dimension; complex (CL-like) fields."""
+    cfg = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=10, fA=0.4)
+    g, o = _pair(B, oracle, cfg, precision=precision)
+    if precision == "f64":
+        _cmp_solve(g, o, 1e-11, 1e-9, True)
+        for which, j in ((0, 1), (0, 10), (1, 1), (1, 7), (1, 10)):
+            assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - o.get_slice(which, j))) < 1e-9, (which, j)
+    else:
+        g.propagate(); o.propagate()
+        Qg, pa, pb = g.density_operators()
+        Qo, oa, ob = o.density_operators()
+        assert abs(Qg - Qo) < 2e-4 * abs(Qo)
+        assert np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 and np.max(np.abs(pb.cpu().numpy() - ob)) < 2e-4
+
+
+@pytest.mark.parametrize("n", [128, 256])
+def test_long_pencils_truncated_march(B, oracle, n):
+    """Pencil lengths 128 and 256 along each dimension in turn (the other two short), 4 contour steps."""
+    for perm in range(3):
+        grid = [8, 8, 16]; grid[perm] = n
+        cfg = inputs.small_diblock(grid=tuple(grid), cell=(3.0, 4.0, 5.0), Ns=10, fA=0.4, seed=perm)
+        g, o = _pair(B, oracle, cfg)
+        g.propagate(4); o.propagate(4)
+        for which in (0, 1):
+            assert np.max(np.abs(g.get_slice(which, 4).cpu().numpy() - o.get_slice(which, 4))) < 1e-10, (grid, which)
+
+
+def test_uniform_field_and_invariants_on_device(B):
+    """Device-only properties that hold at any size: uniform field closed form; mean q_j q+_{Ns-j} = Q; mean phi."""
+    grid, Ns = (32, 32, 32), 20
+    g = B.Fts(grid, (4.0, 4.0, 4.0), Ns, "external")
+    w0 = 0.3 - 1.1j
+    g.set_fields(torch.full(grid, w0, dtype=torch.complex128, device="cuda:0"))
+    g.propagate()
+    Q, phi, _ = g.density_operators()
+    assert abs(Q - np.exp(-w0)) < 1e-13 and float((phi - 1).abs().max()) < 1e-12
+    cfg = inputs.small_diblock(grid=(32, 32, 32), Ns=20, fA=0.4)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", **_kw(cfg))
+    g.set_fields(_dev(cfg.f0), _dev(cfg.f1))
+    g.propagate()
+    Q, pa, pb = g.density_operators()
+    for j in range(0, Ns + 1, 3):
+        Qj = complex((g.get_slice(0, j) * g.get_slice(1, Ns - j)).mean().item())
+        assert abs(Qj - Q) < 1e-12 * abs(Q)
+    assert abs(complex(pa.mean().item()) - cfg.fA) < 1e-12 and abs(complex((pa + pb).mean().item()) - 1) < 1e-12
+
+
+def test_philox_normals_match_oracle(B, oracle):
+    z = B.debug_normals(12345678901234, 7, 1, 2 ** 33 + 5, 4096).cpu().numpy()
+    ref = np.array([oracle.normal(12345678901234, 7, 1, 2 ** 33 + 5 + i) for i in range(4096)])
+    assert np.max(np.abs(z - ref)) < 1e-13          # same Philox integers; libm vs CUDA log/cos differ by ulps
+
+
+@pytest.mark.parametrize("seidel", [0, 1])
+def test_scft_trajectory(B, oracle, seidel):
+    cfg = inputs.config2(grid=(16, 16, 16), Ns=20)
+    cfg.fA = 0.3
+    g, o = _pair(B, oracle, cfg)
+    for it in range(5):
+        Hg, rg = g.scft_step(5.0, 5.0, seidel)
+        Ho, ro = o.scft_step(5.0, 5.0, seidel)
+        assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9, it
+    a, b = g.get_fields(); oa, ob = o.get_fields()
+    assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-9 and np.max(np.abs(b.cpu().numpy() - ob)) < 1e-9
+
+
+@pytest.mark.parametrize("model,scheme", [("diblock", 0), ("diblock", 1), ("edwards", 0), ("edwards", 1)])
+def test_cl_trajectory_10_steps(B, oracle, model, scheme):
+    """Identical Philox noise on both sides: fields agree to 1e-8 after 10 steps (north_star)."""
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4, C=20.0, complex_fields=False)
+    else:
+        cfg = inputs.config4(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10)
+    g, o = _pair(B, oracle, cfg)
+    for step in range(10):
+        g.cl_step(0.01, scheme, 2024, step)
+        o.cl_step(0.01, scheme, 2024, step)
+    a, b = g.get_fields(); oa, ob = o.get_fields()
+    assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-8
+    if model == "diblock":
+        assert np.max(np.abs(b.cpu().numpy() - ob)) < 1e-8
+    assert np.max(np.abs(a.cpu().numpy() - cfg.f0)) > 1e-3      # the fields did move
+
+
+@pytest.mark.parametrize("model", ["edwards", "diblock", "external"])
+def test_operators(B, oracle, model):
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=(16, 16, 16), Ns=10, fA=0.4)
+    elif model == "edwards":
+        cfg = inputs.config4(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10)
+    else:
+        cfg = inputs.config1(Ns=16)
+    g, o = _pair(B, oracle, cfg)
+    g.propagate(); o.propagate()
+    g.density_operators(); o.density_operators()
+    for x, y in zip(g.operators(), o.operators()):
+        assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+
+
+def test_error_codes(B):
+    g = B.Fts((16, 16, 16), (4.0,) * 3, 10, "external")
+    with pytest.raises(B.FtsError) as e:
+        g.propagate()
+    assert e.value.status == 2                         # fields not set
+    g.set_fields(torch.zeros((16, 16, 16), dtype=torch.complex128, device="cuda:0"))
+    with pytest.raises(B.FtsError) as e:
+        g.density_operators()
+    assert e.value.status == 2                         # density before propagate
+    with pytest.raises(B.FtsError) as e:
+        g.cl_step(0.01, 0, 1, 0)
+    assert e.value.status == 6
+    g.set_fields(torch.full((16, 16, 16), float("nan"), dtype=torch.complex128, device="cuda:0"))
+    g.propagate()
+    with pytest.raises(B.FtsError) as e:
+        g.density_operators()
+    assert e.value.status == 5                         # FTS_ENONFINITE
+
+
+def test_determinism(B):
+    cfg = inputs.small_diblock(grid=(32, 16, 16), Ns=10, fA=0.4)
+    outs = []
+    for _ in range(2):
+        g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", **_kw(cfg))
+        g.set_fields(_dev(cfg.f0), _dev(cfg.f1))
+        g.cl_step(0.01, 0, 5, 0)
+        g.propagate()
+        Q, pa, pb = g.density_operators()
+        outs.append((Q, pa.clone(), pb.clone()))
+    assert outs[0][0] == outs[1][0] and torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])
