@@ -106,6 +106,13 @@ fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], 
  * ON THE DEVICE for n consecutive sites starting at site0; out_dev receives n doubles.  For tests. */
 fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream);
 
+/* Measurement aids for bench.py.  fts_debug_fma_peak launches register-resident FMA chains (64 FMAs per thread per
+ * iteration, 148*8 CTAs of 256 threads) and returns the number of FMAs issued, so the caller's own CUDA-event timing
+ * gives the vector fp64/fp32 peak of this GPU; scratch_dev needs 148*8*256*8 bytes.  fts_launch_count returns the
+ * number of kernels this library has launched since it was loaded. */
+fts_status fts_debug_fma_peak(int precision, int iters, void* scratch_dev, size_t scratch_bytes, double* fma_count, void* stream);
+uint64_t fts_launch_count(void);
+
 const char* fts_last_error(const fts_ctx* ctx);
 const char* fts_version(void);
 

@@ -16,7 +16,7 @@ STATUS = {0: "FTS_OK", 1: "FTS_EINVAL", 2: "FTS_ESTATE", 3: "FTS_EWORKSPACE", 4:
 MODELS = {"external": 0, "edwards": 1, "diblock": 2}
 EXPORTS = ["fts_workspace_bytes", "fts_create", "fts_destroy", "fts_set_fields", "fts_get_fields", "fts_propagate",
            "fts_propagate_steps", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
-           "fts_operators", "fts_debug_normals", "fts_last_error", "fts_version"]
+           "fts_operators", "fts_debug_normals", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
 
 
 class FtsParams(C.Structure):
@@ -55,6 +55,8 @@ def lib():
         L.fts_cl_step.argtypes = [vp, C.c_double, C.c_int, C.c_uint64, C.c_uint64, vp]
         L.fts_operators.argtypes = [vp, dp, dp, dp, vp]
         L.fts_debug_normals.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
+        L.fts_debug_fma_peak.argtypes = [C.c_int, C.c_int, vp, C.c_size_t, dp, vp]
+        L.fts_launch_count.restype = C.c_uint64
         L.fts_last_error.argtypes = [vp]
         L.fts_last_error.restype = C.c_char_p
         L.fts_version.restype = C.c_char_p
@@ -168,3 +170,17 @@ def debug_normals(seed, step, field_id, site0, n, device="cuda:0"):
     if rc:
         raise FtsError("fts_debug_normals", rc)
     return out
+
+
+def launch_count():
+    return int(lib().fts_launch_count())
+
+
+def fma_peak_launch(precision, iters, scratch):
+    """Enqueue the FMA-chain kernel on the current stream; returns the FMA count of that launch."""
+    n = C.c_double()
+    rc = lib().fts_debug_fma_peak(0 if precision == "f64" else 1, int(iters), _p(scratch), scratch.numel() * scratch.element_size(),
+                                  C.byref(n), _stream())
+    if rc:
+        raise FtsError("fts_debug_fma_peak", rc)
+    return n.value

@@ -30,6 +30,8 @@ struct Ctx {
     std::string err;
 };
 
+static uint64_t g_launches = 0;      // kernels launched by this library since it was loaded (bench.py's gpu_launches)
+
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Layout {          // the single place that decides where things live in the workspace
@@ -104,6 +106,7 @@ static cudaError_t launch_pass_inst(const PassArgs& A, int njobs, cudaStream_t s
     }
     dim3 grid((A.ntiles + Cfg::GPB - 1) / Cfg::GPB, njobs);
     pass_kernel<T, N, EPT, TZ><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    g_launches += 1;
     return cudaGetLastError();
 }
 template <class T, int TZ>
@@ -153,6 +156,7 @@ static cudaError_t reduce(const Ctx* c, const void* a, const void* b, double p, 
     int nb = (M + RED_THREADS - 1) / RED_THREADS; if (nb > RED_BLOCKS) nb = RED_BLOCKS;
     reduce_partial_kernel<T, OP><<<nb, RED_THREADS, 0, st>>>((const cplx<T>*)a, (const cplx<T>*)b, M, p, c->partial);
     reduce_final_kernel<OP><<<1, 1024, 0, st>>>(c->partial, nb, scale, out_dev);
+    g_launches += 2;
     return cudaGetLastError();
 }
 
@@ -170,8 +174,10 @@ static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
     const size_t M = c->M; const int Ns = c->Ns, np = c->nprop;
     const double ds = 1.0 / Ns;
     boltzmann_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)c->e4[0], (cplx<T>*)c->e4[1], (int)M, c->P.model, ds / 4);
+    g_launches += 1;
     for (int b = 0; b < np; ++b) fill_kernel<T><<<ew_blocks(M), 256, 0, st>>>((cplx<T>*)c->q[b], (int)M, (T)1, (T)0);   // q(x,0) = 1, q+(x,s=1) = 1
     CK(cudaGetLastError());
+    g_launches += np;
     for (int j = 0; j < nsteps; ++j) {
         const void* e4b[2]; const cplx<T>* qin[2]; cplx<T>* qout[2];
         for (int b = 0; b < np; ++b) {
@@ -216,6 +222,7 @@ static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
     const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];              // homopolymer: q+ == q
     density_kernel<T><<<(unsigned)((c->M + 255) / 256), 256, 0, st>>>(q, qd, c->M, c->Ns, c->cA, c->cB, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA,
                                                                        c->nspecies == 2 ? (cplx<T>*)phiB : nullptr);
+    g_launches += 1;
     CK(cudaGetLastError());
     return FTS_OK;
 }
@@ -249,16 +256,19 @@ static fts_status scft_step_t(Ctx* c, double dtp, double dtm, int seidel, double
     CK(cudaMemcpyAsync(c->scal + S_Q0, c->scal + S_Q, 2 * sizeof(double), cudaMemcpyDeviceToDevice, st));
     CK((reduce<T, RED_DIBLOCK_H>(c, c->f0, c->f1, 1.0 / c->P.chiN, 1.0 / (double)M, c->scal + S_H, st)));
     force_plus_kernel<T><<<nb, 256, 0, st>>>((const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M);
+    g_launches += 1;
     CK((reduce<T, RED_MAXABS>(c, c->G[0], nullptr, 0.0, 1.0, c->scal + S_RP, st)));
     Filt f; f.type = FILT_RATIONAL; f.a = dtp; f.b = 0.0; f.c = dtp;                 // dt+/(1 + dt+ g_D(k^2))   (Eq. 11, reading A-10)
     rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
     add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+    g_launches += 1;
     if (seidel) {
         rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
         rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
     }
     scft_minus_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f1, (const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M, (T)(2.0 / c->P.chiN),
                                              (T)(dtm / (1.0 + dtm * 2.0 / c->P.chiN)));
+    g_launches += 1;
     CK((reduce<T, RED_MAXABS>(c, c->G[0], nullptr, 0.0, 1.0, c->scal + S_RM, st)));
     double h[12];
     rc = read_scalars(c, h, 12, st); if (rc) return rc;
@@ -280,22 +290,26 @@ static fts_status cl_step_t(Ctx* c, double dt, int scheme, uint64_t seed, uint64
     if (c->P.model == FTS_MODEL_EDWARDS) {
         const double amp = ns * std::sqrt(2.0 * lp * dt / dV);
         cl_edwards_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->phi[0], (cplx<T>*)c->G[0], M, lp * dt, c->P.B, c->P.C, amp, seed, step, scheme == 0);
+        g_launches += 1;
         CK(cudaGetLastError());
         if (scheme == 1) {
             Filt f; f.type = FILT_RATIONAL; f.a = 1.0; f.b = lp * dt * c->P.B; f.c = lp * dt * c->P.C;
             rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
             add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+            g_launches += 1;
         }
     } else {
         const double ap = ns * std::sqrt(2.0 * lp * dt / dV), am = ns * std::sqrt(2.0 * lm * dt / dV);
         const double dm = scheme == 1 ? 1.0 / (1.0 + lm * dt * 2.0 * c->P.C / c->P.chiN) : 1.0;
         cl_diblock_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (cplx<T>*)c->f1, (const cplx<T>*)c->phi[0], (const cplx<T>*)c->phi[1], (cplx<T>*)c->G[0], M, lp * dt * c->P.C,
                                                  lm * dt * c->P.C, 2.0 / c->P.chiN, ap, am, dm, seed, step, scheme == 0);
+        g_launches += 1;
         CK(cudaGetLastError());
         if (scheme == 1) {
             Filt f; f.type = FILT_RATIONAL; f.a = 1.0; f.b = 0.0; f.c = lp * dt * c->P.C;
             rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
             add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
+            g_launches += 1;
         }
     }
     CK(cudaGetLastError());
@@ -515,10 +529,24 @@ fts_status fts_operators(fts_ctx* c, double H[2], double mu[2], double Pi[2], vo
     return DISPATCH(operators_t<double>(c, H, mu, Pi, st), operators_t<float>(c, H, mu, Pi, st));
 }
 
+// 64 FMAs per thread per iteration; returns the FMA count of the launch so the caller can turn its own event timing into FLOP/s
+fts_status fts_debug_fma_peak(int precision, int iters, void* scratch_dev, size_t scratch_bytes, double* fma_count, void* stream) {
+    const int blocks = 148 * 8, threads = 256;
+    if (!scratch_dev || iters < 1 || scratch_bytes < (size_t)blocks * threads * 8) return FTS_EINVAL;
+    if (precision == FTS_F64) fma_peak_kernel<double><<<blocks, threads, 0, (cudaStream_t)stream>>>((double*)scratch_dev, iters, 0.999999, 1e-7);
+    else fma_peak_kernel<float><<<blocks, threads, 0, (cudaStream_t)stream>>>((float*)scratch_dev, iters, 0.999999f, 1e-7f);
+    g_launches += 1;
+    if (fma_count) *fma_count = (double)blocks * threads * 64.0 * iters;
+    return cudaGetLastError() == cudaSuccess ? FTS_OK : FTS_ECUDA;
+}
+
+uint64_t fts_launch_count(void) { return g_launches; }
+
 fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream) {
     if (!out_dev) return FTS_EINVAL;
     if (n == 0) return FTS_OK;
     normals_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, field_id, site0, n, out_dev);
+    g_launches += 1;
     return cudaGetLastError() == cudaSuccess ? FTS_OK : FTS_ECUDA;
 }
 

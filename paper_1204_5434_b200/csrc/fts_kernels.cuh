@@ -382,5 +382,27 @@ __global__ void cl_edwards_kernel(cplx<T>* om, const cplx<T>* phi, cplx<T>* g0, 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// measurement aid (bench.py): register-resident FMA chains, 8 independent accumulators per thread, so that the
+// roofline's ALU denominator is a number measured on this GPU at the clocks it actually sustains
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) fma_peak_kernel(T* out, int iters, T a, T b) {
+    T x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = (T)(threadIdx.x + i) * (T)1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+        }
+    }
+    T s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace fts
 #endif
