@@ -108,11 +108,15 @@ class Fts:
         self.h = h
 
     def close(self):
-        if getattr(self, "h", None):
-            lib().fts_destroy(self.h)
-            self.h = None
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.fts_destroy(self.h)
+        self.h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:           # interpreter shutdown: module globals may already be gone
+            pass
 
     def _chk(self, rc, what):
         if rc:

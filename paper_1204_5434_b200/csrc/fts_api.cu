@@ -4,6 +4,7 @@
 // the caller's workspace.  No CPU fallback: every arithmetic step of the path is a kernel in fts_kernels.cuh.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -11,6 +12,7 @@
 
 #include "../../include/fts.h"
 #include "fts_kernels.cuh"
+#include "fts_march.cuh"
 
 namespace fts {
 
@@ -27,15 +29,21 @@ struct Ctx {
     double *cA, *cB, *scal, *kacc; double2* partial;
     void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2];
     bool have_fields, have_prop; int marched;
+    // march schedule (fts_march.cuh)
+    Phase* phases;            // device: persistent template at [0], the four per-launch templates at [MARCH_MAXPH * (1..4)]
+    unsigned* counters;       // device: completion counters, then ticket and error flag
+    size_t counters_bytes;
+    int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms;
     std::string err;
 };
 
 static uint64_t g_launches = 0;      // kernels launched by this library since it was loaded (bench.py's gpu_launches)
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+enum { MARCH_MAXCHUNKS = 64 };
 
 struct Layout {          // the single place that decides where things live in the workspace
-    size_t off_tab[3][2], off_tw[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial;
+    size_t off_tab[3][2], off_tw[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
     size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], total;
 };
 static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
@@ -52,6 +60,9 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
     Lo.off_scal = o; o += align_up(64 * sizeof(double));
     Lo.off_kacc = o; o += align_up((size_t)(Ns + 1) * 2 * sizeof(double));
     Lo.off_partial = o; o += align_up(1024 * sizeof(double2));
+    Lo.off_phases = o; o += align_up(5 * MARCH_MAXPH * sizeof(Phase));
+    Lo.counters_bytes = align_up((size_t)2 * (Ns + 1) * (2 + 2 * MARCH_MAXCHUNKS) * sizeof(unsigned)) + 256;
+    Lo.off_counters = o; o += Lo.counters_bytes;
     for (int i = 0; i < 2; ++i) { Lo.off_f[i] = o; o += field; }
     for (int i = 0; i < 2; ++i) { Lo.off_e4[i] = o; o += field; }
     for (int i = 0; i < 2; ++i) { Lo.off_F[i] = o; o += (i < nprop) ? field : 0; }
@@ -63,6 +74,7 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
     return Lo;
 }
 
+static int ept_of(int N) { return (N == 16 || N >= 128) ? 16 : 8; }     // must match the launch_*_n switches
 static bool pow2_ok(int n) { return n >= 8 && n <= 256 && (n & (n - 1)) == 0; }
 
 static fts_status validate(const int grid[3], const double* cell, int Ns, const fts_params* P, int prec) {
@@ -164,52 +176,178 @@ static cudaError_t reduce(const Ctx* c, const void* a, const void* b, double p, 
 enum { S_Q = 0, S_H = 2, S_RP = 4, S_RM = 6, S_SQ = 8, S_Q0 = 10 };
 
 // ------------------------------------------------------------------------------------------------
-// S2-S7: the march.  Per contour step, five fused passes over the {q, q+} batch:
-//   X1: F = Dx[e2 q],  H = Dx'[e4 q]      Y1: F = Dy F, H = Dy' H      Z: F = e2 Dz F, H = Dz'[e2 Dz' H]
-//   Y2: H = Dy' H                          X2: q' = (4 e4 Dx' H - F)/3  -> slice store
-// (D = full-step factor exp(-k_d^2 ds), D' = half-step factor; the three 1-D factors commute.)
+// S2-S7: the march (fts_march.cuh).  Cubic grids: one persistent launch for the whole march, work items in a
+// fixed ticket order with completion counters.  Other grids: the same kernel, one launch per phase kind and
+// round (stream order replaces the counters), instantiated for that dimension's pencil length.
 // ------------------------------------------------------------------------------------------------
+struct MarchInfo { int threads, gpb_s, gpb_c; size_t smem; };
+
+template <class T, int N, int EPT, int TZ>
+static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
+    typedef MarchCfg<T, N, EPT, TZ> Cfg;
+    if (info) { info->threads = Cfg::THREADS; info->gpb_s = Cfg::GPB_S; info->gpb_c = Cfg::GPB_C; info->smem = Cfg::SMEM; }
+    if (query && !occ) return cudaSuccess;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(march_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    if (occ) {
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<T, N, EPT, TZ>, Cfg::THREADS, Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+    }
+    if (query) return cudaSuccess;
+    march_kernel<T, N, EPT, TZ><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    g_launches += 1;
+    return cudaGetLastError();
+}
+template <class T, int TZ>
+static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
+    switch (N) {
+        case 8: return launch_march_inst<T, 8, 8, TZ>(A, grid, query, info, occ, st);
+        case 16: return launch_march_inst<T, 16, 16, TZ>(A, grid, query, info, occ, st);
+        case 32: return launch_march_inst<T, 32, 8, TZ>(A, grid, query, info, occ, st);
+        case 64: return launch_march_inst<T, 64, 8, TZ>(A, grid, query, info, occ, st);
+        case 128: return launch_march_inst<T, 128, 16, TZ>(A, grid, query, info, occ, st);
+        case 256: return launch_march_inst<T, 256, 16, TZ>(A, grid, query, info, occ, st);
+    }
+    return cudaErrorInvalidValue;
+}
+// tz: pencils per strided tile = complex elements per 128-byte row, or 8 when Nz is shorter than that (complex64, Nz = 8)
+template <class T>
+static cudaError_t launch_march(const Ctx* c, int N, const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
+    constexpr int TZ = tz_of<T>();
+    if (c->g[2] >= TZ) return launch_march_n<T, TZ>(N, A, grid, query, info, occ, st);
+    return launch_march_n<T, 8>(N, A, grid, query, info, occ, st);
+}
+template <class T> static int tz_used(const Ctx* c) { return c->g[2] >= tz_of<T>() ? tz_of<T>() : 8; }
+
+static int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+static Phase mkphase(int first, int kind, int b, int prev, int chunk) {
+    Phase p; p.first = first; p.chunk = (short)chunk; p.kind = (signed char)kind; p.prop_off = (signed char)(b | (prev << 1));
+    return p;
+}
+
+// Ticket counts of one T phase and of one slab's Y1 / Z / Y2 phase for the instantiation `mi`.
+static void phase_counts(const Ctx* c, const MarchInfo& mx, const MarchInfo& my, const MarchInfo& mz, int tz, int planes, int cnt[4]) {
+    const int Ny = c->g[1], Nz = c->g[2];
+    cnt[PH_T] = ceil_div(Ny * Nz / tz, mx.gpb_s);
+    cnt[PH_Y1] = 2 * ceil_div(planes * (Nz / tz), my.gpb_s);
+    cnt[PH_Z] = 2 * ceil_div(planes * Ny, mz.gpb_c);
+    cnt[PH_Y2] = ceil_div(planes * (Nz / tz), my.gpb_s);
+}
+
+// Round template of the persistent march.  Two propagators:  T(q,j) | U(q+,j-1) | U(q,j) | T(q+,j)  so that every
+// whole-field dependency (T -> U of the same step, U -> T of the next) is separated by a block of the other
+// propagator's items.  U = the slabs' Y1, Z, Y2 phases software-pipelined `lag` slabs apart.
+static std::vector<Phase> make_template(int nprop, int nchunks, int lag, const int cnt[4], int* tickets) {
+    std::vector<Phase> v; int first = 0;
+    auto add = [&](int kind, int b, int prev, int chunk) { v.push_back(mkphase(first, kind, b, prev, chunk)); first += cnt[kind]; };
+    auto ublock = [&](int b, int prev) {
+        for (int i = 0; i < nchunks + 2 * lag; ++i) {
+            if (i < nchunks) add(PH_Y1, b, prev, i);
+            if (i - lag >= 0 && i - lag < nchunks) add(PH_Z, b, prev, i - lag);
+            if (i - 2 * lag >= 0 && i - 2 * lag < nchunks) add(PH_Y2, b, prev, i - 2 * lag);
+        }
+    };
+    add(PH_T, 0, 0, 0);
+    if (nprop == 2) ublock(1, 1);
+    ublock(0, 0);
+    if (nprop == 2) add(PH_T, 1, 0, 0);
+    *tickets = first;
+    return v;
+}
+
+template <class T>
+static void fill_march_args(const Ctx* c, MarchArgs& A, int nsteps) {
+    std::memset(&A, 0, sizeof A);
+    for (int b = 0; b < 2; ++b) { A.q[b] = c->q[b]; A.F[b] = c->F[b]; A.H[b] = c->H[b]; A.e4[b] = c->e4[b]; }
+    for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; A.tw[d] = c->dim[d].tw; A.g[d] = c->g[d]; }
+    A.M = (long long)c->M; A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nsteps = nsteps;
+    A.done = c->counters; A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
+}
+
+// Decide the schedule once per context (needs the device: occupancy, SM count) and upload the templates.
+template <class T>
+static fts_status plan_march(Ctx* c) {
+    const int Nx = c->g[0], Ny = c->g[1], Nz = c->g[2], tz = tz_used<T>(c);
+    MarchArgs A; fill_march_args<T>(c, A, 0);
+    MarchInfo mi[3];
+    for (int d = 0; d < 3; ++d) CK(launch_march<T>(c, c->g[d], A, 0, true, &mi[d], nullptr, 0));
+    int dev = 0; CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
+    const char* mode = std::getenv("FTS_MARCH");
+    c->persistent = (Nx == Ny && Ny == Nz) && !(mode && std::strcmp(mode, "launch") == 0);
+    // slab size: F and H of both propagators of `lag`-many slabs in flight must sit in L2 next to the streaming traffic
+    const size_t plane = (size_t)Ny * Nz * c->esz;
+    size_t target = (size_t)4 << 20;
+    if (const char* e = std::getenv("FTS_SLAB_BYTES")) target = (size_t)std::atoll(e);
+    int planes = Nx;
+    while (planes > 1 && (size_t)planes * plane > target) planes >>= 1;
+    while (Nx / planes > MARCH_MAXCHUNKS) planes <<= 1;
+    if (!c->persistent) planes = Nx;
+    c->planes = planes; c->nchunks = Nx / planes;
+    c->lag = 1;
+    if (const char* e = std::getenv("FTS_LAG")) c->lag = std::atoi(e) > 0 ? std::atoi(e) : 1;
+    std::vector<Phase> all(5 * MARCH_MAXPH, mkphase(0, 0, 0, 0, 0));
+    if (c->persistent) {
+        phase_counts(c, mi[0], mi[1], mi[2], tz, planes, c->cnt);
+        std::vector<Phase> t = make_template(c->nprop, c->nchunks, c->lag, c->cnt, &c->tickets_per_round);
+        if ((int)t.size() > MARCH_MAXPH) { c->err = "march template too long"; return FTS_EINVAL; }
+        c->nph = (int)t.size();
+        std::copy(t.begin(), t.end(), all.begin());
+    }
+    // per-launch templates (stream-ordered mode): kind k at all[MARCH_MAXPH*(1+k)], one phase per propagator
+    int cl[4]; phase_counts(c, mi[0], mi[1], mi[2], tz, Nx, cl);
+    for (int k = 0; k < 4; ++k)
+        for (int b = 0; b < c->nprop; ++b) all[MARCH_MAXPH * (1 + k) + b] = mkphase(b * cl[k], k, b, 0, 0);
+    if (!c->persistent) for (int k = 0; k < 4; ++k) c->cnt[k] = cl[k];
+    CK(cudaMemcpy(c->phases, all.data(), all.size() * sizeof(Phase), cudaMemcpyHostToDevice));
+    return FTS_OK;
+}
+
+template <class T>
+static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
+    MarchArgs A; fill_march_args<T>(c, A, nsteps);
+    CK(cudaMemsetAsync(c->counters, 0, c->counters_bytes - 128, st));          // counters and ticket; the error flag is sticky
+    if (c->persistent) {
+        A.nchunks = c->nchunks; A.planes = c->planes;
+        A.phases = c->phases; A.nphases = c->nph; A.tickets_per_round = c->tickets_per_round; A.round0 = 0; A.round1 = nsteps;
+        A.ntT = c->cnt[PH_T]; A.nY1 = c->cnt[PH_Y1]; A.nZ = c->cnt[PH_Z]; A.nY2 = c->cnt[PH_Y2];
+        A.ticket = (unsigned*)((char*)c->counters + c->counters_bytes - 256);
+        int occ = 0; MarchInfo mi;
+        CK(launch_march<T>(c, c->g[0], A, 0, true, &mi, &occ, st));
+        if (occ < 1) { c->err = "march kernel does not fit on an SM"; return FTS_ECUDA; }
+        long long total = (long long)(nsteps + 1) * c->tickets_per_round;
+        long long grid = (long long)occ * c->sms;
+        if (grid > total) grid = total;
+        CK(launch_march<T>(c, c->g[0], A, (int)grid, false, nullptr, nullptr, st));
+        return FTS_OK;
+    }
+    A.nchunks = 1; A.planes = c->g[0]; A.ticket = nullptr;
+    A.ntT = c->cnt[PH_T]; A.nY1 = c->cnt[PH_Y1]; A.nZ = c->cnt[PH_Z]; A.nY2 = c->cnt[PH_Y2];
+    static const int dim_of[4] = {0, 1, 2, 1};
+    for (int j = 0; j <= nsteps; ++j) {
+        for (int k = 0; k < 4; ++k) {
+            if (k != PH_T && j == nsteps) break;
+            A.phases = c->phases + MARCH_MAXPH * (1 + k); A.nphases = c->nprop; A.tickets_per_round = c->nprop * c->cnt[k];
+            A.round0 = A.round1 = j;
+            CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
+        }
+    }
+    return FTS_OK;
+}
+
 template <class T>
 static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
-    const size_t M = c->M; const int Ns = c->Ns, np = c->nprop;
+    const size_t M = c->M; const int Ns = c->Ns;
     const double ds = 1.0 / Ns;
     boltzmann_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)c->e4[0], (cplx<T>*)c->e4[1], (int)M, c->P.model, ds / 4);
     g_launches += 1;
-    for (int b = 0; b < np; ++b) fill_kernel<T><<<ew_blocks(M), 256, 0, st>>>((cplx<T>*)c->q[b], (int)M, (T)1, (T)0);   // q(x,0) = 1, q+(x,s=1) = 1
     CK(cudaGetLastError());
-    g_launches += np;
-    for (int j = 0; j < nsteps; ++j) {
-        const void* e4b[2]; const cplx<T>* qin[2]; cplx<T>* qout[2];
-        for (int b = 0; b < np; ++b) {
-            int sp = 0;
-            if (c->nspecies == 2) sp = (b == 0) ? (j >= c->jA ? 1 : 0) : (j < Ns - c->jA ? 1 : 0);      // O5 / O6 species schedule
-            e4b[b] = c->e4[sp];
-            qin[b] = (const cplx<T>*)c->q[b] + (size_t)j * M;
-            qout[b] = (cplx<T>*)c->q[b] + (size_t)(j + 1) * M;
-        }
-        PassArgs A; std::memset(&A, 0, sizeof A);
-        int n = 0;
-        for (int b = 0; b < np; ++b) {
-            A.job[n++] = mkjob(qin[b], c->F[b], OP_D, PRE_E2, 0, e4b[b]);
-            A.job[n++] = mkjob(qin[b], c->H[b], OP_D, PRE_E4, 1, e4b[b]);
-        }
-        CK(launch_pass<T>(c, 0, A, n, st));
-        n = 0;
-        for (int b = 0; b < np; ++b) { A.job[n++] = mkjob(c->F[b], c->F[b], OP_D, PRE_NONE, 0); A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1); }
-        CK(launch_pass<T>(c, 1, A, n, st));
-        n = 0;
-        for (int b = 0; b < np; ++b) {
-            A.job[n++] = mkjob(c->F[b], c->F[b], OP_D, PRE_NONE, 0, e4b[b], 0, 0, POST_E2);
-            A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1, e4b[b], 1, 1);
-        }
-        CK(launch_pass<T>(c, 2, A, n, st));
-        n = 0;
-        for (int b = 0; b < np; ++b) A.job[n++] = mkjob(c->H[b], c->H[b], OP_D, PRE_NONE, 1);
-        CK(launch_pass<T>(c, 1, A, n, st));
-        n = 0;
-        for (int b = 0; b < np; ++b) A.job[n++] = mkjob(c->H[b], qout[b], OP_D, PRE_NONE, 1, e4b[b], 0, 0, POST_COMBINE, c->F[b]);
-        CK(launch_pass<T>(c, 0, A, n, st));
-    }
+    fts_status rc = march_t<T>(c, nsteps, st); if (rc) return rc;
     // S7 (Eq. 4): Q = (1/M) sum_x q_Ns(x), fixed-order tree
     CK((reduce<T, RED_SUM>(c, (const cplx<T>*)c->q[0] + (size_t)nsteps * M, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st)));
     c->marched = nsteps; c->have_prop = true;
@@ -243,8 +381,11 @@ static fts_status filter3d_t(Ctx* c, void* g, Filt f, cudaStream_t st) {
 }
 
 static fts_status read_scalars(Ctx* c, double* host, int n, cudaStream_t st) {
+    int flag = 0;
     CK(cudaMemcpyAsync(host, c->scal, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&flag, (char*)c->counters + c->counters_bytes - 128, sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    if (flag) { c->err = "march kernel: a dependency wait timed out (results invalid)"; return FTS_ECUDA; }
     return FTS_OK;
 }
 
@@ -390,9 +531,13 @@ static fts_status build_tables(Ctx* c) {
             k2[i] = (double)(k * k);
             t0[i] = (T)((double)std::exp(-(k * k) * (long double)ds) / (double)N);             // inverse-FFT 1/N folded in
             t1[i] = (T)((double)std::exp(-(k * k) * (long double)ds * 0.5L) / (double)N);
-            const long double a = -2.0L * kPiL * (long double)i / (long double)N;
-            tw[i] = mk<T>((T)std::cos(a), (T)std::sin(a));
         }
+        const int ept = ept_of(N), tpp = N / ept;              // twiddles per (register r, thread t): exp(-2 pi i t r / N)
+        for (int r = 0; r < ept && tpp > 1; ++r)
+            for (int t = 0; t < tpp; ++t) {
+                const long double a = -2.0L * kPiL * (long double)(((long)t * r) % N) / (long double)N;
+                tw[r * tpp + t] = mk<T>((T)std::cos(a), (T)std::sin(a));
+            }
         CK(cudaMemcpy(c->dim[d].tab[0], t0.data(), N * sizeof(T), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].tab[1], t1.data(), N * sizeof(T), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].tw, tw.data(), N * sizeof(cplx<T>), cudaMemcpyHostToDevice));
@@ -403,6 +548,7 @@ static fts_status build_tables(Ctx* c) {
     CK(cudaMemcpy(c->cA, wA.data(), wA.size() * sizeof(double), cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->cB, wB.data(), wB.size() * sizeof(double), cudaMemcpyHostToDevice));
     CK(cudaMemset(c->scal, 0, 64 * sizeof(double)));
+    CK(cudaMemset(c->counters, 0, c->counters_bytes));
     return FTS_OK;
 }
 
@@ -452,8 +598,10 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
         c->e4[i] = c->ws + Lo.off_e4[i]; c->F[i] = c->ws + Lo.off_F[i]; c->H[i] = c->ws + Lo.off_H[i];
         c->q[i] = c->ws + Lo.off_q[i]; c->phi[i] = c->ws + Lo.off_phi[i]; c->G[i] = c->ws + Lo.off_G[i];
     }
+    c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->have_fields = c->have_prop = false; c->marched = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
+    if (!rc) rc = DISPATCH(plan_march<double>(c), plan_march<float>(c));
     if (rc) { delete c; return rc; }
     *out = c;
     return FTS_OK;

@@ -1,0 +1,413 @@
+// fts_march.cuh — the contour march as ONE persistent kernel per propagator solve.
+//
+// One RQM4 step (Eq. 12) of a propagator is split into four kinds of work items, each a fused
+// 1-D pass over a tile of pencils held in registers (fts_pencil.h):
+//
+//   T  (x pencils)  finish step s-1:  q_s = (4 e4 Dx'[H] - F)/3  -> slice store;   start step s:  F = Dx[e2 q_s], H = Dx'[e4 q_s]
+//   Y1 (y pencils)  F = Dy F,  H = Dy' H
+//   Z  (z pencils)  F = e2 Dz F,  H = Dz'[e2 Dz' H]
+//   Y2 (y pencils)  H = Dy' H
+//
+// (D = exp(ds d^2/dx_d^2) applied as FFT -> real table -> IFFT along one dimension, D' the same at ds/2; the three
+// 1-D factors of exp(-k^2 ds) commute, so the half branch is ordered x y z | z y x and its two z diffusions meet
+// around the real-space multiply.)  F and H are updated in place.  Per step and propagator the items move
+// 6 (T) + 4 (Y1) + 5 (Z) + 2 (Y2) fields through L2; Y1, Z and Y2 are issued slab by slab over x-ranges small
+// enough that a slab of F and H stays resident in the 126 MB L2 from its Y1 read to its Y2 write, so HBM sees
+// about 11 field transfers per step instead of 17.
+//
+// Scheduling: work items are handed out in a fixed global order through an atomic ticket; an item waits (acquire
+// poll on a per-phase completion counter) for the phase it depends on, which always precedes it in ticket order, so
+// the kernel is deadlock-free for any grid size.  The q and q+ marches are independent; their phases are
+// interleaved half a step apart so that the whole-field dependency T <-> {Y1,Z,Y2} of one propagator is always
+// separated by a block of the other propagator's work.  Data crosses CTAs only through L2: every field access is
+// ld.global.cg / st.global.cg.
+#ifndef FTS_MARCH_CUH
+#define FTS_MARCH_CUH
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fts_pencil.h"
+
+namespace fts {
+
+enum { PH_T = 0, PH_Y1 = 1, PH_Z = 2, PH_Y2 = 3 };
+enum { MARCH_MAXPH = 512 };
+
+struct Phase {              // one entry of the round template ("round" j holds the phases listed in make_template)
+    int first;              // first ticket of the phase inside the round
+    short chunk;            // x-slab index (Y1, Z, Y2)
+    signed char kind;       // PH_*
+    signed char prop_off;   // bit 0: propagator b; bit 1: the phase belongs to step (round - 1)
+};
+
+struct MarchArgs {
+    void* q[2]; void* F[2]; void* H[2]; const void* e4[2];
+    const void* tab[3][2];      // per dimension: exp(-k_d^2 ds)/N_d, exp(-k_d^2 ds/2)/N_d
+    const void* tw[3];          // per dimension: inter-stage twiddles, per-(register, thread) layout
+    int g[3];
+    long long M;
+    int Ns, jA, nspecies, nsteps;
+    int nchunks, planes;        // x-slabs and planes per slab
+    const Phase* phases; int nphases; int tickets_per_round; int round0, round1;   // rounds [round0, round1]
+    int ntT, nY1, nZ, nY2;      // tickets of one T phase / of one slab's Y1, Z, Y2 phase
+    unsigned* ticket;           // NULL: one item per CTA (ticket = blockIdx.x) and no dependency waits (stream order)
+    unsigned* done;             // completion counters [prop][step][2 + 2*nchunks]: T, Y2 (all slabs), Y1[slab], Z[slab]
+    int* err;                   // set to 1 if a dependency wait timed out
+};
+
+template <class T> struct vec2;
+template <> struct vec2<double> { typedef double2 type; };
+template <> struct vec2<float> { typedef float2 type; };
+
+template <class T> __device__ __forceinline__ cplx<T> ldcg(const cplx<T>* p) {
+    typename vec2<T>::type v = __ldcg(reinterpret_cast<const typename vec2<T>::type*>(p));
+    return mk<T>(v.x, v.y);
+}
+template <class T> __device__ __forceinline__ void stcg(cplx<T>* p, cplx<T> v) {
+    typename vec2<T>::type w; w.x = v.x; w.y = v.y;
+    __stcg(reinterpret_cast<typename vec2<T>::type*>(p), w);
+}
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+template <class T, int N, int EPT, int TZ>
+struct MarchCfg {
+    typedef PencilShape<N, EPT> S;
+    static constexpr int TARGET = 128;
+    static constexpr int GROUP_S = TZ * S::TPP;                                       // threads of one strided tile [N][TZ]
+    static constexpr int GPB_S = (TARGET / GROUP_S) > 0 ? (TARGET / GROUP_S) : 1;     // strided tiles per item
+    static constexpr int THREADS = GROUP_S * GPB_S;
+    static constexpr int GPB_C = THREADS / S::TPP;                                    // contiguous pencils per item
+    static constexpr int PS = contig_ps<T, N, EPT>();
+    static constexpr int XELEMS = S::ONE ? 1 : ((GPB_C * PS > GPB_S * N * TZ) ? GPB_C * PS : GPB_S * N * TZ);
+    typedef XchgLayout<PS, S::R2 + 1, 1> LC;
+    typedef XchgLayout<1, S::R2 * TZ, TZ> LS;
+    static constexpr size_t SMEM = (size_t)N * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T) + (size_t)XELEMS * sizeof(cplx<T>) +
+                                   2 * (size_t)THREADS * EPT * sizeof(cplx<T>) + (size_t)MARCH_MAXPH * sizeof(Phase);
+    static constexpr int MINB = (sizeof(T) == 8 && EPT == 16) ? 2 : ((THREADS <= 128) ? 3 : 2);
+};
+
+// exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform.
+// One shared-memory buffer serves both exchanges: every thread overwrites only what it last read.  `contig`
+// (block-uniform) selects the exchange addressing of the z pass (LC) or of the x/y passes (LS); the butterflies are shared.
+template <class T, int N, int EPT, class LS, class LC>
+__device__ __forceinline__ void diffuse(cplx<T> (&v)[EPT], int t, int p, bool contig, const cplx<T>* s_tw, const T* tab, cplx<T>* xs, cplx<T>* xc) {
+    typedef Pencil<T, N, EPT> P;
+    typedef PencilShape<N, EPT> S;
+    P::fwd_a(v, t, s_tw);
+    if constexpr (!S::ONE) {
+        if (contig) P::template xchg_store_a<LC>(v, t, xc, p); else P::template xchg_store_a<LS>(v, t, xs, p);
+        __syncthreads();
+        if (contig) P::template xchg_load_b<LC>(v, t, xc, p); else P::template xchg_load_b<LS>(v, t, xs, p);
+    }
+    P::fwd_b(v);
+#pragma unroll
+    for (int r = 0; r < EPT; ++r) v[r] = v[r] * tab[t + S::TPP * r];
+    P::inv_b(v);
+    if constexpr (!S::ONE) {
+        if (contig) P::template xchg_store_b<LC>(v, t, xc, p); else P::template xchg_store_b<LS>(v, t, xs, p);
+        __syncthreads();
+        if (contig) P::template xchg_load_a<LC>(v, t, xc, p); else P::template xchg_load_a<LS>(v, t, xs, p);
+    }
+    P::inv_a(v, t, s_tw);
+}
+
+// cp.async of one complex element (generic proxy, so ordinary acquire/release ordering applies): 16 bytes bypass L1;
+// 8 bytes (complex64) go through L1, which the dependency acquire of the item has invalidated.
+template <class T> __device__ __forceinline__ void cp_async_elem(cplx<T>* smem_dst, const cplx<T>* gsrc) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if constexpr (sizeof(T) == 8) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NLEFT> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT) : "memory"); }
+
+template <class T>
+struct Item {                 // one work item, as seen by one thread
+    int kind, job, s, b, chunk, state;      // state 0: end of march, 1: work, 2: ticket of a phase outside the march
+    int t, p, xoff;
+    bool contig, active;
+    long long base0, estride;               // pencil point of register r is base0 + r*estride
+    const cplx<T>* src;                     // primary input field (H for T items)
+};
+
+template <class T, int N, int EPT, int TZ>
+__global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, N, EPT, TZ>::MINB) march_kernel(const MarchArgs A) {
+    typedef MarchCfg<T, N, EPT, TZ> Cfg;
+    typedef typename Cfg::S S;
+    typedef typename Cfg::LS LS;
+    typedef typename Cfg::LC LC;
+    typedef cplx<T> C;
+    constexpr int TPP = S::TPP;
+    constexpr int NT = Cfg::THREADS;
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* s_tw = reinterpret_cast<C*>(smem_raw);
+    T* s_tab = reinterpret_cast<T*>(s_tw + N);
+    C* s_x = reinterpret_cast<C*>(s_tab + 2 * N);          // exchange buffer of the transforms
+    C* s_stash = s_x + Cfg::XELEMS;                        // thread-private [r][tid]: e4 tile, then the stashed half-branch input
+    C* s_pre = s_stash + NT * EPT;                         // thread-private [r][tid]: primary input of the NEXT item (and F of a T item)
+    Phase* s_ph = reinterpret_cast<Phase*>(s_pre + NT * EPT);
+    __shared__ int s_item[2][6];              // step, phase index, index inside the phase, state, dependency ready
+
+    const int tid = threadIdx.x;
+    for (int i = tid; i < A.nphases; i += NT) s_ph[i] = A.phases[i];
+    int cur_dim = -1;
+    const int C2 = 2 + 2 * A.nchunks;         // counters per (propagator, step)
+    const long long total = (long long)(A.round1 - A.round0 + 1) * A.tickets_per_round;
+    const int Ny = A.g[1], Nz = A.g[2];
+    const int two = A.nspecies == 2;
+    __syncthreads();
+
+    // the completion counter an item of (phase, step) waits for, and the count it needs
+    auto dependency = [&](const Phase& ph, int s, unsigned& need) -> const unsigned* {
+        const int b = ph.prop_off & 1;
+        const unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
+        need = 0;
+        if (ph.kind == PH_T) { if (s <= 0) return nullptr; need = (unsigned)(A.nchunks * A.nY2); return cnt - C2 + 1; }
+        if (ph.kind == PH_Y1) { need = (unsigned)A.ntT; return cnt; }
+        if (ph.kind == PH_Z) { need = (unsigned)A.nY1; return cnt + 2 + ph.chunk; }
+        need = (unsigned)A.nZ; return cnt + 2 + A.nchunks + ph.chunk;
+    };
+    // thread 0: take the next ticket, decode it into s_item[slot], test its dependency without blocking
+    auto fetch = [&](int slot, bool first) {
+        const long long tk = A.ticket ? (long long)atomicAdd(A.ticket, 1u) : (first ? (long long)blockIdx.x : total);
+        int state = tk < total ? 1 : 0, ready = 1;
+        if (state) {
+            const int round = A.round0 + (int)(tk / A.tickets_per_round), off = (int)(tk % A.tickets_per_round);
+            int lo = 0, hi = A.nphases - 1;
+            while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_ph[mid].first <= off) lo = mid; else hi = mid - 1; }
+            const Phase ph = s_ph[lo];
+            const int s = round - ((ph.prop_off >> 1) & 1);
+            const bool live = ph.kind == PH_T ? (s >= 0 && s <= A.nsteps) : (s >= 0 && s < A.nsteps);
+            s_item[slot][0] = s; s_item[slot][1] = lo; s_item[slot][2] = off - ph.first;
+            if (!live) state = 2;
+            else if (A.ticket) {
+                unsigned need; const unsigned* w = dependency(ph, s, need);
+                if (w && ld_acquire(w) < need) ready = 0;
+            }
+        }
+        s_item[slot][3] = state; s_item[slot][4] = ready;
+    };
+    // every thread: its coordinates inside the item published in s_item[slot]
+    auto decode = [&](int slot, Item<T>& I, Phase& ph) {
+        I.state = s_item[slot][3];
+        if (I.state != 1) return;
+        I.s = s_item[slot][0];
+        ph = s_ph[s_item[slot][1]];
+        const int idx = s_item[slot][2];
+        I.b = ph.prop_off & 1; I.kind = ph.kind; I.chunk = ph.chunk; I.job = 0; I.xoff = 0;
+        I.contig = I.kind == PH_Z;
+        if (I.contig) {                                               // GPB_C pencils per item, lanes run along the pencil
+            const int per_job = A.nZ >> 1;
+            I.job = idx / per_job;
+            I.t = tid % TPP; I.p = tid / TPP;
+            const int local = (idx - I.job * per_job) * Cfg::GPB_C + I.p;
+            I.active = local < A.planes * Ny;
+            I.base0 = ((long long)I.chunk * A.planes * Ny + local) * N + I.t;
+            I.estride = TPP;
+        } else {                                                      // tiles [N][TZ], lanes run along z (the contiguous direction)
+            const int zz = tid % TZ, tb = tid / (TZ * TPP);
+            I.t = (tid / TZ) % TPP; I.p = zz; I.xoff = tb * (N * TZ);
+            if (I.kind == PH_T) {
+                const int tile = idx * Cfg::GPB_S + tb;
+                I.active = tile < (Ny * Nz) / TZ;
+                const long long ps = (long long)Ny * Nz;
+                I.base0 = (long long)tile * TZ + zz + I.t * ps;
+                I.estride = ps * TPP;
+            } else {
+                const int tpp_z = Nz / TZ;                            // tiles per plane
+                int tg = idx;
+                I.job = 1;
+                if (I.kind == PH_Y1) { const int per_job = A.nY1 >> 1; I.job = idx / per_job; tg = idx - I.job * per_job; }
+                const int local = tg * Cfg::GPB_S + tb;
+                I.active = local < A.planes * tpp_z;
+                const int tile = I.chunk * A.planes * tpp_z + local;
+                I.base0 = (long long)(tile / tpp_z) * Ny * Nz + (long long)(tile % tpp_z) * TZ + zz + (long long)I.t * Nz;
+                I.estride = (long long)Nz * TPP;
+            }
+        }
+        I.src = static_cast<const C*>((I.kind == PH_T || I.job == 1) ? A.H[I.b] : A.F[I.b]);
+    };
+    auto has_primary = [&](const Item<T>& I) { return !(I.kind == PH_T && I.s == 0); };
+    auto prefetch_tile = [&](C* dst, const C* src, const Item<T>& I) {      // this thread's EPT points -> dst[r][tid]
+        if (I.active) {
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) cp_async_elem<T>(dst + r * NT + tid, src + I.base0 + r * I.estride);
+        }
+        cp_async_commit();
+    };
+
+    Item<T> cur, nxt;
+    Phase cph, nph;
+    int slot = 0;
+    if (tid == 0) fetch(0, true);
+    __syncthreads();
+    decode(0, cur, cph);
+    bool cur_ready = s_item[0][4] != 0, cur_pref = false;
+
+    while (cur.state != 0) {
+        // ---- look one item ahead (ticket, coordinates, is its dependency already met?) ----
+        if (tid == 0) {
+            fetch(slot ^ 1, false);
+            if (cur.state == 1 && !cur_ready && A.ticket) {           // blocking wait for the current item's dependency
+                unsigned need; const unsigned* w = dependency(cph, cur.s, need);
+                unsigned spins = 0;
+                while (w && ld_acquire(w) < need) {
+                    __nanosleep(100);
+                    if (++spins > (1u << 23)) { atomicExch(A.err, 1); break; }       // never hang the GPU: flag it and carry on
+                }
+            }
+        }
+        __syncthreads();
+        decode(slot ^ 1, nxt, nph);
+        const bool nxt_ready = s_item[slot ^ 1][4] != 0;
+        bool nxt_pref = false;
+
+        if (cur.state == 1) {
+            const int kind = cur.kind, job = cur.job, s = cur.s, b = cur.b;
+            const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
+            if (dim != cur_dim) {
+                for (int i = tid; i < N; i += NT) {
+                    s_tw[i] = static_cast<const C*>(A.tw[dim])[i];
+                    s_tab[i] = static_cast<const T*>(A.tab[dim][0])[i];
+                    s_tab[N + i] = static_cast<const T*>(A.tab[dim][1])[i];
+                }
+                cur_dim = dim;
+                __syncthreads();
+            }
+            // species of a contour step (O5 / O6 block schedule)
+            const int sp_now = !two ? 0 : (b == 0 ? (s >= A.jA ? 1 : 0) : (s < A.Ns - A.jA ? 1 : 0));
+            const int sp_prev = !two ? 0 : (b == 0 ? (s - 1 >= A.jA ? 1 : 0) : (s - 1 < A.Ns - A.jA ? 1 : 0));
+            C* Fb = static_cast<C*>(A.F[b]);
+            C* Hb = static_cast<C*>(A.H[b]);
+            const bool active = cur.active;
+            const long long base0 = cur.base0, estride = cur.estride;
+            const bool finish = s > 0, start = s < A.nsteps;          // T items only
+            C* xs = s_x + cur.xoff;
+            C v[EPT];
+
+            // secondary input e4 -> s_stash, needed after the first diffusion (T finish, Z)
+            const bool e4_staged = (kind == PH_T && finish) || kind == PH_Z;
+            if (e4_staged) prefetch_tile(s_stash, static_cast<const C*>(A.e4[kind == PH_T ? sp_prev : sp_now]), cur);
+            // primary input: staged by the previous iteration, or loaded directly
+            if (has_primary(cur)) {
+                if (cur_pref) {
+                    if (e4_staged) cp_async_wait<1>(); else cp_async_wait<0>();
+#pragma unroll
+                    for (int r = 0; r < EPT; ++r) v[r] = s_pre[r * NT + tid];
+                } else {
+#pragma unroll
+                    for (int r = 0; r < EPT; ++r) v[r] = active ? ldcg(cur.src + base0 + r * estride) : mk<T>(0, 0);
+                }
+            }
+            // s_pre is free again: T items stage F for the combine, the others stage the next item's primary input now
+            auto stage_next = [&]() {
+                if (nxt.state == 1 && nxt_ready && has_primary(nxt)) { prefetch_tile(s_pre, nxt.src, nxt); nxt_pref = true; }
+            };
+            if (kind == PH_T) { if (finish) prefetch_tile(s_pre, Fb, cur); }
+            else stage_next();
+
+            // T item tail: from q_s in v, write the slice, then b = e4 q_s -> stash, a = e4 b -> v   (start of step s)
+            auto emit_q_and_start = [&](bool combine) {
+                C* qs = static_cast<C*>(A.q[b]) + (long long)s * A.M;
+                const C* e4s = static_cast<const C*>(A.e4[sp_now]);
+                const bool reload = !combine || sp_now != sp_prev;
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) {
+                    const long long i = base0 + r * estride;
+                    C e = mk<T>(0, 0);
+                    if (combine) {                                    // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
+                        e = s_stash[r * NT + tid];
+                        const C f = s_pre[r * NT + tid];
+                        const C h = v[r] * e;
+                        v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
+                    }
+                    if (active) stcg(qs + i, v[r]);                   // the slice store IS the step's output write
+                    if (start) {
+                        if (reload) e = active ? ldcg(e4s + i) : mk<T>(0, 0);
+                        const C hb = v[r] * e;
+                        s_stash[r * NT + tid] = hb;
+                        v[r] = hb * e;
+                    }
+                }
+            };
+
+            int st = 0;
+            if (kind == PH_T && !finish) {                            // q(x,0) = 1, q+(x,s=1) = 1
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
+                emit_q_and_start(false);
+                stage_next();
+                st = 1;
+            }
+#pragma unroll 1
+            for (;;) {
+                // table of this diffusion: full step for the F branch (T stage 1, job 0), half step otherwise
+                const bool full = kind == PH_T ? (st == 1) : (job == 0);
+                diffuse<T, N, EPT, LS, LC>(v, cur.t, cur.p, cur.contig, s_tw, full ? s_tab : s_tab + N, xs, s_x);
+                if (kind == PH_T) {
+                    if (st == 0) {
+                        cp_async_wait<0>();                           // e4 and F tiles of this item
+                        emit_q_and_start(true);
+                        stage_next();
+                        if (!start) break;
+                        st = 1;
+                    } else if (st == 1) {
+                        if (active) {
+#pragma unroll
+                            for (int r = 0; r < EPT; ++r) stcg(Fb + base0 + r * estride, v[r]);
+                        }
+#pragma unroll
+                        for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
+                        st = 2;
+                    } else {
+                        if (active) {
+#pragma unroll
+                            for (int r = 0; r < EPT; ++r) stcg(Hb + base0 + r * estride, v[r]);
+                        }
+                        break;
+                    }
+                } else if (kind == PH_Z && st == 0) {                 // F = e2 Dz F;  H = Dz'[e2 Dz' H]
+                    if (nxt_pref) cp_async_wait<1>(); else cp_async_wait<0>();      // the e4 tile (committed before the next item's tile)
+#pragma unroll
+                    for (int r = 0; r < EPT; ++r) {
+                        const C e = s_stash[r * NT + tid];
+                        v[r] = v[r] * (e * e);
+                    }
+                    if (job == 0) {
+                        if (active) {
+#pragma unroll
+                            for (int r = 0; r < EPT; ++r) stcg(Fb + base0 + r * estride, v[r]);
+                        }
+                        break;
+                    }
+                    st = 1;
+                } else {                                              // Y1, Y2, second z diffusion of H
+                    C* dst = job == 0 ? Fb : Hb;
+                    if (active) {
+#pragma unroll
+                        for (int r = 0; r < EPT; ++r) stcg(dst + base0 + r * estride, v[r]);
+                    }
+                    break;
+                }
+            }
+        }
+        __syncthreads();                      // all stores of the item are issued
+        if (tid == 0 && cur.state == 1 && A.ticket) {
+            unsigned* cnt = A.done + ((size_t)cur.b * (A.Ns + 1) + cur.s) * C2;
+            unsigned* c = cur.kind == PH_T ? cnt : cur.kind == PH_Y2 ? cnt + 1 : cur.kind == PH_Y1 ? cnt + 2 + cur.chunk : cnt + 2 + A.nchunks + cur.chunk;
+            __threadfence();
+            atomicAdd(c, 1u);
+        }
+        cur = nxt; cph = nph; cur_ready = nxt_ready; cur_pref = nxt_pref; slot ^= 1;
+    }
+    cp_async_wait<0>();
+}
+
+}  // namespace fts
+#endif

@@ -131,7 +131,9 @@ struct Pencil {
     typedef PencilShape<N, EPT> S;
     typedef cplx<T> C;
 
-    // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.  tw[m] = exp(-2 pi i m / N).
+    // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.  The twiddles are stored per
+    // (register, thread): tw[r*TPP + t] = exp(-2 pi i (t + TPP*g) k1 / N) with g = r % G1, k1 = r / G1, so that the
+    // lanes of a warp read consecutive (contiguous pass) or identical (strided pass) addresses.
     template <class TW>
     static FTS_HD void fwd_a(C (&v)[EPT], int t, const TW* tw) {
         static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, -1>(v); });
@@ -139,7 +141,7 @@ struct Pencil {
             static_for<0, EPT>([&](auto rr) {
                 constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
                 if constexpr (k1 > 0) {
-                    TW w = tw[(t + S::TPP * g) * k1];
+                    TW w = tw[r * S::TPP + t];
                     v[r] = v[r] * mk<T>((T)w.x, (T)w.y);
                 }
             });
@@ -192,7 +194,7 @@ struct Pencil {
             static_for<0, EPT>([&](auto rr) {
                 constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
                 if constexpr (k1 > 0) {
-                    TW w = tw[(t + S::TPP * g) * k1];
+                    TW w = tw[r * S::TPP + t];
                     v[r] = v[r] * mk<T>((T)w.x, -(T)w.y);
                 }
             });

@@ -23,9 +23,14 @@ void run(int npencil, double tol) {
     constexpr int PS_contig = contig_ps<T, N, EPT>();
     typedef typename std::conditional<strided, XchgLayout<1, S::R2 * TZ, TZ>, XchgLayout<PS_contig, S::R2 + 1, 1>>::type L;
     size_t smn = strided ? (size_t)N * TZ : (size_t)npencil * PS_contig + N + 64;
-    std::vector<cplx<T>> sm(smn + 1024), tw(N);
+    std::vector<cplx<T>> sm(smn + 1024), tw(N);       // tw: per-(register, thread) layout of fts_pencil.h
     std::vector<cplx<double>> twd(N);
-    for (int m = 0; m < N; ++m) { double a = -2 * M_PI * m / N; twd[m] = mk<double>(cos(a), sin(a)); tw[m] = mk<T>((T)cos(a), (T)sin(a)); }
+    for (int m = 0; m < N; ++m) { double a = -2 * M_PI * m / N; twd[m] = mk<double>(cos(a), sin(a)); }
+    for (int r = 0; r < EPT; ++r) for (int t = 0; t < TPP; ++t) {
+        const int g = r % S::G1, k1 = r / S::G1;
+        double a = -2 * M_PI * (((long)(t + TPP * g) * k1) % N) / N;
+        tw[r * TPP + t] = mk<T>((T)cos(a), (T)sin(a));
+    }
     std::vector<std::vector<cd>> x(npencil, std::vector<cd>(N));
     srand(N * 131 + EPT);
     for (auto& p : x) for (auto& e : p) e = cd(rand() / (double)RAND_MAX - 0.5, rand() / (double)RAND_MAX - 0.5);
