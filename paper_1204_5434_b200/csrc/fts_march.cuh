@@ -126,13 +126,13 @@ template <class T> __device__ __forceinline__ void cp_async_elem(cplx<T>* smem_d
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NLEFT> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NLEFT) : "memory"); }
 
+// Coordinates of one thread inside a work item.  Recomputed from the item descriptor in shared memory wherever they are
+// needed (a few integer instructions) instead of being kept live across the transforms, where they would spill.
 template <class T>
-struct Item {                 // one work item, as seen by one thread
-    int kind, job, s, b, chunk, state;      // state 0: end of march, 1: work, 2: ticket of a phase outside the march
-    int t, p, xoff;
-    bool contig, active;
-    long long base0, estride;               // pencil point of register r is base0 + r*estride
-    const cplx<T>* src;                     // primary input field (H for T items)
+struct Coords {
+    int kind, job, s, b, chunk;
+    bool active;
+    int base0, estride;                     // element offset of register r inside a field: base0 + r*estride   (M <= 2^24)
 };
 
 template <class T, int N, int EPT, int TZ>
@@ -152,15 +152,14 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
     C* s_stash = s_x + Cfg::XELEMS;                        // thread-private [r][tid]: e4 tile, then the stashed half-branch input
     C* s_pre = s_stash + NT * EPT;                         // thread-private [r][tid]: primary input of the NEXT item (and F of a T item)
     Phase* s_ph = reinterpret_cast<Phase*>(s_pre + NT * EPT);
-    __shared__ int s_item[2][6];              // step, phase index, index inside the phase, state, dependency ready
+    __shared__ int s_item[2][8];              // step, phase index, index inside the phase, state, dependency ready
+    __shared__ int s_dim;                     // dimension whose tables are loaded
 
     const int tid = threadIdx.x;
     for (int i = tid; i < A.nphases; i += NT) s_ph[i] = A.phases[i];
-    int cur_dim = -1;
+    if (tid == 0) s_dim = -1;
     const int C2 = 2 + 2 * A.nchunks;         // counters per (propagator, step)
-    const long long total = (long long)(A.round1 - A.round0 + 1) * A.tickets_per_round;
-    const int Ny = A.g[1], Nz = A.g[2];
-    const int two = A.nspecies == 2;
+    const unsigned total = (unsigned)((A.round1 - A.round0 + 1) * A.tickets_per_round);
     __syncthreads();
 
     // the completion counter an item of (phase, step) waits for, and the count it needs
@@ -173,153 +172,160 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
         if (ph.kind == PH_Z) { need = (unsigned)A.nY1; return cnt + 2 + ph.chunk; }
         need = (unsigned)A.nZ; return cnt + 2 + A.nchunks + ph.chunk;
     };
-    // thread 0: take the next ticket, decode it into s_item[slot], test its dependency without blocking
-    auto fetch = [&](int slot, bool first) {
-        const long long tk = A.ticket ? (long long)atomicAdd(A.ticket, 1u) : (first ? (long long)blockIdx.x : total);
+    // thread 0: decode the ticket drawn one iteration ago into s_item[slot], draw the next one (its latency hides behind
+    // the current item), test the dependency without blocking.  A counter once seen complete stays complete.
+    unsigned tk_pending = 0;
+    const unsigned* dep_ok = nullptr;
+    if (tid == 0) tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : blockIdx.x;
+    auto fetch = [&](int slot) {
+        const unsigned tk = tk_pending;
+        tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : total;
         int state = tk < total ? 1 : 0, ready = 1;
         if (state) {
-            const int round = A.round0 + (int)(tk / A.tickets_per_round), off = (int)(tk % A.tickets_per_round);
+            const int round = A.round0 + (int)(tk / (unsigned)A.tickets_per_round), off = (int)(tk % (unsigned)A.tickets_per_round);
             int lo = 0, hi = A.nphases - 1;
             while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_ph[mid].first <= off) lo = mid; else hi = mid - 1; }
             const Phase ph = s_ph[lo];
             const int s = round - ((ph.prop_off >> 1) & 1);
             const bool live = ph.kind == PH_T ? (s >= 0 && s <= A.nsteps) : (s >= 0 && s < A.nsteps);
             s_item[slot][0] = s; s_item[slot][1] = lo; s_item[slot][2] = off - ph.first;
-            if (!live) state = 2;
+            if (!live) state = 2;                                       // ticket of a phase outside the march: no work
             else if (A.ticket) {
                 unsigned need; const unsigned* w = dependency(ph, s, need);
-                if (w && ld_acquire(w) < need) ready = 0;
+                if (w && w != dep_ok) { if (ld_acquire(w) < need) ready = 0; else dep_ok = w; }
             }
         }
         s_item[slot][3] = state; s_item[slot][4] = ready;
     };
     // every thread: its coordinates inside the item published in s_item[slot]
-    auto decode = [&](int slot, Item<T>& I, Phase& ph) {
-        I.state = s_item[slot][3];
-        if (I.state != 1) return;
-        I.s = s_item[slot][0];
-        ph = s_ph[s_item[slot][1]];
-        const int idx = s_item[slot][2];
-        I.b = ph.prop_off & 1; I.kind = ph.kind; I.chunk = ph.chunk; I.job = 0; I.xoff = 0;
-        I.contig = I.kind == PH_Z;
-        if (I.contig) {                                               // GPB_C pencils per item, lanes run along the pencil
+    const int Ny = A.g[1], Nz = A.g[2];
+    auto coords = [&](int slot, Coords<T>& c) {
+        const volatile int* it = s_item[slot];
+        c.s = it[0];
+        const Phase ph = s_ph[it[1]];
+        const int idx = it[2];
+        c.b = ph.prop_off & 1; c.kind = ph.kind; c.chunk = ph.chunk; c.job = 0;
+        if (c.kind == PH_Z) {                                         // GPB_C pencils per item, lanes run along the pencil
             const int per_job = A.nZ >> 1;
-            I.job = idx / per_job;
-            I.t = tid % TPP; I.p = tid / TPP;
-            const int local = (idx - I.job * per_job) * Cfg::GPB_C + I.p;
-            I.active = local < A.planes * Ny;
-            I.base0 = ((long long)I.chunk * A.planes * Ny + local) * N + I.t;
-            I.estride = TPP;
+            c.job = idx >= per_job;
+            const int local = (idx - c.job * per_job) * Cfg::GPB_C + tid / TPP;
+            c.active = local < A.planes * Ny;
+            c.base0 = (c.chunk * A.planes * Ny + local) * N + tid % TPP;
+            c.estride = TPP;
         } else {                                                      // tiles [N][TZ], lanes run along z (the contiguous direction)
-            const int zz = tid % TZ, tb = tid / (TZ * TPP);
-            I.t = (tid / TZ) % TPP; I.p = zz; I.xoff = tb * (N * TZ);
-            if (I.kind == PH_T) {
+            const int zz = tid % TZ, tb = tid / (TZ * TPP), t = (tid / TZ) % TPP;
+            if (c.kind == PH_T) {
                 const int tile = idx * Cfg::GPB_S + tb;
-                I.active = tile < (Ny * Nz) / TZ;
-                const long long ps = (long long)Ny * Nz;
-                I.base0 = (long long)tile * TZ + zz + I.t * ps;
-                I.estride = ps * TPP;
+                c.active = tile < (Ny * Nz) / TZ;
+                c.base0 = tile * TZ + zz + t * (Ny * Nz);
+                c.estride = Ny * Nz * TPP;
             } else {
-                const int tpp_z = Nz / TZ;                            // tiles per plane
+                const int tpp_z = Nz / TZ, lg = 31 - __clz(tpp_z);    // tiles per plane (a power of two)
                 int tg = idx;
-                I.job = 1;
-                if (I.kind == PH_Y1) { const int per_job = A.nY1 >> 1; I.job = idx / per_job; tg = idx - I.job * per_job; }
+                c.job = 1;
+                if (c.kind == PH_Y1) { const int per_job = A.nY1 >> 1; c.job = idx >= per_job; tg = idx - c.job * per_job; }
                 const int local = tg * Cfg::GPB_S + tb;
-                I.active = local < A.planes * tpp_z;
-                const int tile = I.chunk * A.planes * tpp_z + local;
-                I.base0 = (long long)(tile / tpp_z) * Ny * Nz + (long long)(tile % tpp_z) * TZ + zz + (long long)I.t * Nz;
-                I.estride = (long long)Nz * TPP;
+                c.active = local < A.planes * tpp_z;
+                const int tile = c.chunk * A.planes * tpp_z + local;
+                c.base0 = (tile >> lg) * Ny * Nz + (tile & (tpp_z - 1)) * TZ + zz + t * Nz;
+                c.estride = Nz * TPP;
             }
         }
-        I.src = static_cast<const C*>((I.kind == PH_T || I.job == 1) ? A.H[I.b] : A.F[I.b]);
     };
-    auto has_primary = [&](const Item<T>& I) { return !(I.kind == PH_T && I.s == 0); };
-    auto prefetch_tile = [&](C* dst, const C* src, const Item<T>& I) {      // this thread's EPT points -> dst[r][tid]
-        if (I.active) {
+    auto primary_src = [&](const Coords<T>& c) { return static_cast<const C*>((c.kind == PH_T || c.job == 1) ? A.H[c.b] : A.F[c.b]); };
+    auto prefetch_tile = [&](C* dst, const C* src, const Coords<T>& c) {      // this thread's EPT points -> dst[r][tid]
+        if (c.active) {
 #pragma unroll
-            for (int r = 0; r < EPT; ++r) cp_async_elem<T>(dst + r * NT + tid, src + I.base0 + r * I.estride);
+            for (int r = 0; r < EPT; ++r) cp_async_elem<T>(dst + r * NT + tid, src + c.base0 + r * c.estride);
         }
         cp_async_commit();
     };
+    // species of contour step `step` of propagator b (O5 / O6 block schedule)
+    auto species = [&](int b, int step) -> int {
+        if (A.nspecies != 2) return 0;
+        return b == 0 ? (step >= A.jA ? 1 : 0) : (step < A.Ns - A.jA ? 1 : 0);
+    };
 
-    Item<T> cur, nxt;
-    Phase cph, nph;
-    int slot = 0;
-    if (tid == 0) fetch(0, true);
+    int slot = 0, cur_dim = -1;
+    bool cur_pref = false;
+    if (tid == 0) fetch(0);
     __syncthreads();
-    decode(0, cur, cph);
-    bool cur_ready = s_item[0][4] != 0, cur_pref = false;
 
-    while (cur.state != 0) {
-        // ---- look one item ahead (ticket, coordinates, is its dependency already met?) ----
+    for (;;) {
+        const int state = ((const volatile int*)s_item[slot])[3];
+        if (state == 0) break;
+        // ---- look one item ahead; block on the current item's dependency only if it was not met when it was drawn ----
         if (tid == 0) {
-            fetch(slot ^ 1, false);
-            if (cur.state == 1 && !cur_ready && A.ticket) {           // blocking wait for the current item's dependency
-                unsigned need; const unsigned* w = dependency(cph, cur.s, need);
+            fetch(slot ^ 1);
+            if (state == 1 && s_item[slot][4] == 0 && A.ticket) {
+                const Phase ph = s_ph[s_item[slot][1]];
+                unsigned need; const unsigned* w = dependency(ph, s_item[slot][0], need);
                 unsigned spins = 0;
                 while (w && ld_acquire(w) < need) {
                     __nanosleep(100);
                     if (++spins > (1u << 23)) { atomicExch(A.err, 1); break; }       // never hang the GPU: flag it and carry on
                 }
+                dep_ok = w;
             }
         }
         __syncthreads();
-        decode(slot ^ 1, nxt, nph);
-        const bool nxt_ready = s_item[slot ^ 1][4] != 0;
         bool nxt_pref = false;
-
-        if (cur.state == 1) {
-            const int kind = cur.kind, job = cur.job, s = cur.s, b = cur.b;
-            const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
-            if (dim != cur_dim) {
-                for (int i = tid; i < N; i += NT) {
-                    s_tw[i] = static_cast<const C*>(A.tw[dim])[i];
-                    s_tab[i] = static_cast<const T*>(A.tab[dim][0])[i];
-                    s_tab[N + i] = static_cast<const T*>(A.tab[dim][1])[i];
-                }
-                cur_dim = dim;
-                __syncthreads();
+        // stage the next item's primary input into s_pre (only if its dependency is already met)
+        auto stage_next = [&]() {
+            const volatile int* nx = s_item[slot ^ 1];
+            if (nx[3] == 1 && nx[4] != 0) {
+                Coords<T> n; coords(slot ^ 1, n);
+                if (!(n.kind == PH_T && n.s == 0)) { prefetch_tile(s_pre, primary_src(n), n); nxt_pref = true; }
             }
-            // species of a contour step (O5 / O6 block schedule)
-            const int sp_now = !two ? 0 : (b == 0 ? (s >= A.jA ? 1 : 0) : (s < A.Ns - A.jA ? 1 : 0));
-            const int sp_prev = !two ? 0 : (b == 0 ? (s - 1 >= A.jA ? 1 : 0) : (s - 1 < A.Ns - A.jA ? 1 : 0));
-            C* Fb = static_cast<C*>(A.F[b]);
-            C* Hb = static_cast<C*>(A.H[b]);
-            const bool active = cur.active;
-            const long long base0 = cur.base0, estride = cur.estride;
-            const bool finish = s > 0, start = s < A.nsteps;          // T items only
-            C* xs = s_x + cur.xoff;
+        };
+
+        if (state == 1) {
             C v[EPT];
-
-            // secondary input e4 -> s_stash, needed after the first diffusion (T finish, Z)
-            const bool e4_staged = (kind == PH_T && finish) || kind == PH_Z;
-            if (e4_staged) prefetch_tile(s_stash, static_cast<const C*>(A.e4[kind == PH_T ? sp_prev : sp_now]), cur);
-            // primary input: staged by the previous iteration, or loaded directly
-            if (has_primary(cur)) {
-                if (cur_pref) {
-                    if (e4_staged) cp_async_wait<1>(); else cp_async_wait<0>();
-#pragma unroll
-                    for (int r = 0; r < EPT; ++r) v[r] = s_pre[r * NT + tid];
-                } else {
-#pragma unroll
-                    for (int r = 0; r < EPT; ++r) v[r] = active ? ldcg(cur.src + base0 + r * estride) : mk<T>(0, 0);
+            int kind, st = 0;
+            bool contig;
+            {   // ---- load phase ----
+                Coords<T> c; coords(slot, c);
+                kind = c.kind; contig = kind == PH_Z;
+                const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
+                if (dim != cur_dim) {
+                    for (int i = tid; i < N; i += NT) {
+                        s_tw[i] = static_cast<const C*>(A.tw[dim])[i];
+                        s_tab[i] = static_cast<const T*>(A.tab[dim][0])[i];
+                        s_tab[N + i] = static_cast<const T*>(A.tab[dim][1])[i];
+                    }
+                    cur_dim = dim;
+                    __syncthreads();
                 }
+                const bool finish = c.s > 0;
+                // secondary input e4 -> s_stash, needed after the first diffusion (T finish, Z)
+                const bool e4_staged = (kind == PH_T && finish) || kind == PH_Z;
+                if (e4_staged) prefetch_tile(s_stash, static_cast<const C*>(A.e4[species(c.b, kind == PH_T ? c.s - 1 : c.s)]), c);
+                if (!(kind == PH_T && !finish)) {                     // primary input: staged by the previous iteration, or loaded directly
+                    if (cur_pref) {
+                        if (e4_staged) cp_async_wait<1>(); else cp_async_wait<0>();
+#pragma unroll
+                        for (int r = 0; r < EPT; ++r) v[r] = s_pre[r * NT + tid];
+                    } else {
+                        const C* src = primary_src(c);
+#pragma unroll
+                        for (int r = 0; r < EPT; ++r) v[r] = c.active ? ldcg(src + c.base0 + r * c.estride) : mk<T>(0, 0);
+                    }
+                }
+                // s_pre is free again: T items stage F for the combine, the others stage the next item's primary input now
+                if (kind == PH_T) { if (finish) prefetch_tile(s_pre, static_cast<const C*>(A.F[c.b]), c); }
+                else stage_next();
             }
-            // s_pre is free again: T items stage F for the combine, the others stage the next item's primary input now
-            auto stage_next = [&]() {
-                if (nxt.state == 1 && nxt_ready && has_primary(nxt)) { prefetch_tile(s_pre, nxt.src, nxt); nxt_pref = true; }
-            };
-            if (kind == PH_T) { if (finish) prefetch_tile(s_pre, Fb, cur); }
-            else stage_next();
-
             // T item tail: from q_s in v, write the slice, then b = e4 q_s -> stash, a = e4 b -> v   (start of step s)
             auto emit_q_and_start = [&](bool combine) {
-                C* qs = static_cast<C*>(A.q[b]) + (long long)s * A.M;
+                Coords<T> c; coords(slot, c);
+                const bool start = c.s < A.nsteps;
+                const int sp_now = species(c.b, c.s), sp_prev = species(c.b, c.s - 1);
+                C* qs = static_cast<C*>(A.q[c.b]) + (long long)c.s * A.M;
                 const C* e4s = static_cast<const C*>(A.e4[sp_now]);
                 const bool reload = !combine || sp_now != sp_prev;
 #pragma unroll
                 for (int r = 0; r < EPT; ++r) {
-                    const long long i = base0 + r * estride;
+                    const int i = c.base0 + r * c.estride;
                     C e = mk<T>(0, 0);
                     if (combine) {                                    // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
                         e = s_stash[r * NT + tid];
@@ -327,49 +333,60 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
                         const C h = v[r] * e;
                         v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                     }
-                    if (active) stcg(qs + i, v[r]);                   // the slice store IS the step's output write
+                    if (c.active) stcg(qs + i, v[r]);                 // the slice store IS the step's output write
                     if (start) {
-                        if (reload) e = active ? ldcg(e4s + i) : mk<T>(0, 0);
+                        if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
                         const C hb = v[r] * e;
                         s_stash[r * NT + tid] = hb;
                         v[r] = hb * e;
                     }
                 }
+                return start;
+            };
+            auto store_tile = [&](int which) {                        // 0: F, 1: H of the item's propagator
+                Coords<T> c; coords(slot, c);
+                C* dst = static_cast<C*>(which ? A.H[c.b] : A.F[c.b]);
+                if (c.active) {
+#pragma unroll
+                    for (int r = 0; r < EPT; ++r) stcg(dst + c.base0 + r * c.estride, v[r]);
+                }
+                return c.job;
             };
 
-            int st = 0;
-            if (kind == PH_T && !finish) {                            // q(x,0) = 1, q+(x,s=1) = 1
+            int job = 0;
+            if (kind == PH_T) {
+                if (((const volatile int*)s_item[slot])[0] == 0) {    // q(x,0) = 1, q+(x,s=1) = 1
 #pragma unroll
-                for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
-                emit_q_and_start(false);
-                stage_next();
-                st = 1;
+                    for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
+                    emit_q_and_start(false);
+                    stage_next();
+                    st = 1;
+                }
+            } else {
+                Coords<T> c; coords(slot, c);
+                job = c.job;
             }
 #pragma unroll 1
             for (;;) {
-                // table of this diffusion: full step for the F branch (T stage 1, job 0), half step otherwise
+                // thread position inside the transform, and the table: full step for the F branch, half step otherwise
+                const int t = contig ? tid % TPP : (tid / TZ) % TPP, p = contig ? tid / TPP : tid % TZ;
+                C* xs = contig ? s_x : s_x + (tid / (TZ * TPP)) * (N * TZ);
                 const bool full = kind == PH_T ? (st == 1) : (job == 0);
-                diffuse<T, N, EPT, LS, LC>(v, cur.t, cur.p, cur.contig, s_tw, full ? s_tab : s_tab + N, xs, s_x);
+                diffuse<T, N, EPT, LS, LC>(v, t, p, contig, s_tw, full ? s_tab : s_tab + N, xs, s_x);
                 if (kind == PH_T) {
                     if (st == 0) {
                         cp_async_wait<0>();                           // e4 and F tiles of this item
-                        emit_q_and_start(true);
+                        const bool start = emit_q_and_start(true);
                         stage_next();
                         if (!start) break;
                         st = 1;
                     } else if (st == 1) {
-                        if (active) {
-#pragma unroll
-                            for (int r = 0; r < EPT; ++r) stcg(Fb + base0 + r * estride, v[r]);
-                        }
+                        store_tile(0);
 #pragma unroll
                         for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
                         st = 2;
                     } else {
-                        if (active) {
-#pragma unroll
-                            for (int r = 0; r < EPT; ++r) stcg(Hb + base0 + r * estride, v[r]);
-                        }
+                        store_tile(1);
                         break;
                     }
                 } else if (kind == PH_Z && st == 0) {                 // F = e2 Dz F;  H = Dz'[e2 Dz' H]
@@ -379,32 +396,24 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
                         const C e = s_stash[r * NT + tid];
                         v[r] = v[r] * (e * e);
                     }
-                    if (job == 0) {
-                        if (active) {
-#pragma unroll
-                            for (int r = 0; r < EPT; ++r) stcg(Fb + base0 + r * estride, v[r]);
-                        }
-                        break;
-                    }
+                    if (job == 0) { store_tile(0); break; }
                     st = 1;
                 } else {                                              // Y1, Y2, second z diffusion of H
-                    C* dst = job == 0 ? Fb : Hb;
-                    if (active) {
-#pragma unroll
-                        for (int r = 0; r < EPT; ++r) stcg(dst + base0 + r * estride, v[r]);
-                    }
+                    store_tile(job);
                     break;
                 }
             }
         }
         __syncthreads();                      // all stores of the item are issued
-        if (tid == 0 && cur.state == 1 && A.ticket) {
-            unsigned* cnt = A.done + ((size_t)cur.b * (A.Ns + 1) + cur.s) * C2;
-            unsigned* c = cur.kind == PH_T ? cnt : cur.kind == PH_Y2 ? cnt + 1 : cur.kind == PH_Y1 ? cnt + 2 + cur.chunk : cnt + 2 + A.nchunks + cur.chunk;
+        if (tid == 0 && state == 1 && A.ticket) {
+            const Phase ph = s_ph[s_item[slot][1]];
+            const int b = ph.prop_off & 1, s = s_item[slot][0];
+            unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
+            unsigned* c = ph.kind == PH_T ? cnt : ph.kind == PH_Y2 ? cnt + 1 : ph.kind == PH_Y1 ? cnt + 2 + ph.chunk : cnt + 2 + A.nchunks + ph.chunk;
             __threadfence();
             atomicAdd(c, 1u);
         }
-        cur = nxt; cph = nph; cur_ready = nxt_ready; cur_pref = nxt_pref; slot ^= 1;
+        cur_pref = nxt_pref; slot ^= 1;
     }
     cp_async_wait<0>();
 }
