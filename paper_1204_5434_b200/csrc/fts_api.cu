@@ -185,7 +185,7 @@ struct MarchInfo { int threads, gpb_s, gpb_c; size_t smem; };
 template <class T, int N, int EPT, int TZ>
 static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
     typedef MarchCfg<T, N, EPT, TZ> Cfg;
-    if (info) { info->threads = Cfg::THREADS; info->gpb_s = Cfg::GPB_S; info->gpb_c = Cfg::GPB_C; info->smem = Cfg::SMEM; }
+    if (info) { info->threads = Cfg::LAUNCH; info->gpb_s = Cfg::GPB_S; info->gpb_c = Cfg::GPB_C; info->smem = Cfg::SMEM; }
     if (query && !occ) return cudaSuccess;
     static bool attr_done = false;
     if (!attr_done) {
@@ -194,11 +194,11 @@ static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, M
         attr_done = true;
     }
     if (occ) {
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<T, N, EPT, TZ>, Cfg::THREADS, Cfg::SMEM);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<T, N, EPT, TZ>, Cfg::LAUNCH, Cfg::SMEM);
         if (e != cudaSuccess) return e;
     }
     if (query) return cudaSuccess;
-    march_kernel<T, N, EPT, TZ><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    march_kernel<T, N, EPT, TZ><<<grid, Cfg::LAUNCH, Cfg::SMEM, st>>>(A);
     g_launches += 1;
     return cudaGetLastError();
 }

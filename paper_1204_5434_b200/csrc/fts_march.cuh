@@ -88,20 +88,46 @@ struct MarchCfg {
     typedef XchgLayout<1, S::R2 * TZ, TZ> LS;
     static constexpr size_t SMEM = (size_t)N * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T) + (size_t)XELEMS * sizeof(cplx<T>) +
                                    2 * (size_t)THREADS * EPT * sizeof(cplx<T>) + (size_t)MARCH_MAXPH * sizeof(Phase);
+    static constexpr int LAUNCH = THREADS + 32;                                       // + one scheduler warp
     static constexpr int MINB = (sizeof(T) == 8 && EPT == 16) ? 2 : ((THREADS <= 128) ? 3 : 2);
 };
+
+// barrier among the NT compute threads of a CTA (the scheduler warp does not take part)
+template <int NT> __device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); }
+
+// mbarrier primitives (shared memory, CTA scope): the scheduler warp and the compute warps hand items back and forth
+__device__ __forceinline__ void mbar_init(uint64_t* b, unsigned count) {
+    asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("{ .reg .b64 st; mbarrier.arrive.shared.b64 st, [%0]; }" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint64_t* b, unsigned parity) {
+    unsigned ok;
+    asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ bool mbar_wait(uint64_t* b, unsigned parity) {      // false: gave up (never hang the GPU)
+    unsigned ok, tries = 0;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+    } while (!ok && ++tries < (1u << 24));
+    return ok != 0;
+}
 
 // exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform.
 // One shared-memory buffer serves both exchanges: every thread overwrites only what it last read.  `contig`
 // (block-uniform) selects the exchange addressing of the z pass (LC) or of the x/y passes (LS); the butterflies are shared.
-template <class T, int N, int EPT, class LS, class LC>
+template <class T, int N, int EPT, int NT, class LS, class LC>
 __device__ __forceinline__ void diffuse(cplx<T> (&v)[EPT], int t, int p, bool contig, const cplx<T>* s_tw, const T* tab, cplx<T>* xs, cplx<T>* xc) {
     typedef Pencil<T, N, EPT> P;
     typedef PencilShape<N, EPT> S;
     P::fwd_a(v, t, s_tw);
     if constexpr (!S::ONE) {
         if (contig) P::template xchg_store_a<LC>(v, t, xc, p); else P::template xchg_store_a<LS>(v, t, xs, p);
-        __syncthreads();
+        bar_compute<NT>();
         if (contig) P::template xchg_load_b<LC>(v, t, xc, p); else P::template xchg_load_b<LS>(v, t, xs, p);
     }
     P::fwd_b(v);
@@ -110,7 +136,7 @@ __device__ __forceinline__ void diffuse(cplx<T> (&v)[EPT], int t, int p, bool co
     P::inv_b(v);
     if constexpr (!S::ONE) {
         if (contig) P::template xchg_store_b<LC>(v, t, xc, p); else P::template xchg_store_b<LS>(v, t, xs, p);
-        __syncthreads();
+        bar_compute<NT>();
         if (contig) P::template xchg_load_a<LC>(v, t, xc, p); else P::template xchg_load_a<LS>(v, t, xs, p);
     }
     P::inv_a(v, t, s_tw);
@@ -135,15 +161,18 @@ struct Coords {
     int base0, estride;                     // element offset of register r inside a field: base0 + r*estride   (M <= 2^24)
 };
 
+enum { MARCH_RING = 4 };      // item descriptors in flight between the scheduler warp and the compute warps
+
 template <class T, int N, int EPT, int TZ>
-__global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, N, EPT, TZ>::MINB) march_kernel(const MarchArgs A) {
+__global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N, EPT, TZ>::MINB) march_kernel(const MarchArgs A) {
     typedef MarchCfg<T, N, EPT, TZ> Cfg;
     typedef typename Cfg::S S;
     typedef typename Cfg::LS LS;
     typedef typename Cfg::LC LC;
     typedef cplx<T> C;
     constexpr int TPP = S::TPP;
-    constexpr int NT = Cfg::THREADS;
+    constexpr int NT = Cfg::THREADS;          // compute threads; warp NT/32 is the scheduler
+    constexpr int R = MARCH_RING;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* s_tw = reinterpret_cast<C*>(smem_raw);
@@ -152,51 +181,95 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
     C* s_stash = s_x + Cfg::XELEMS;                        // thread-private [r][tid]: e4 tile, then the stashed half-branch input
     C* s_pre = s_stash + NT * EPT;                         // thread-private [r][tid]: primary input of the NEXT item (and F of a T item)
     Phase* s_ph = reinterpret_cast<Phase*>(s_pre + NT * EPT);
-    __shared__ int s_item[2][8];              // step, phase index, index inside the phase, state, dependency ready
-    __shared__ int s_dim;                     // dimension whose tables are loaded
+    __shared__ int s_item[R][4];              // step, phase index, index inside the phase, state (0: end of march, 1: work)
+    __shared__ __align__(8) uint64_t s_full[R], s_done[R];
 
     const int tid = threadIdx.x;
-    for (int i = tid; i < A.nphases; i += NT) s_ph[i] = A.phases[i];
-    if (tid == 0) s_dim = -1;
+    for (int i = tid; i < A.nphases; i += Cfg::LAUNCH) s_ph[i] = A.phases[i];
+    if (tid == 0) {
+        for (int i = 0; i < R; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_done[i], NT); }
+    }
     const int C2 = 2 + 2 * A.nchunks;         // counters per (propagator, step)
     const unsigned total = (unsigned)((A.round1 - A.round0 + 1) * A.tickets_per_round);
     __syncthreads();
 
-    // the completion counter an item of (phase, step) waits for, and the count it needs
-    auto dependency = [&](const Phase& ph, int s, unsigned& need) -> const unsigned* {
-        const int b = ph.prop_off & 1;
-        const unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
-        need = 0;
-        if (ph.kind == PH_T) { if (s <= 0) return nullptr; need = (unsigned)(A.nchunks * A.nY2); return cnt - C2 + 1; }
-        if (ph.kind == PH_Y1) { need = (unsigned)A.ntT; return cnt; }
-        if (ph.kind == PH_Z) { need = (unsigned)A.nY1; return cnt + 2 + ph.chunk; }
-        need = (unsigned)A.nZ; return cnt + 2 + A.nchunks + ph.chunk;
-    };
-    // thread 0: decode the ticket drawn one iteration ago into s_item[slot], draw the next one (its latency hides behind
-    // the current item), test the dependency without blocking.  A counter once seen complete stays complete.
-    unsigned tk_pending = 0;
-    const unsigned* dep_ok = nullptr;
-    if (tid == 0) tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : blockIdx.x;
-    auto fetch = [&](int slot) {
-        const unsigned tk = tk_pending;
-        tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : total;
-        int state = tk < total ? 1 : 0, ready = 1;
-        if (state) {
-            const int round = A.round0 + (int)(tk / (unsigned)A.tickets_per_round), off = (int)(tk % (unsigned)A.tickets_per_round);
-            int lo = 0, hi = A.nphases - 1;
-            while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_ph[mid].first <= off) lo = mid; else hi = mid - 1; }
-            const Phase ph = s_ph[lo];
-            const int s = round - ((ph.prop_off >> 1) & 1);
-            const bool live = ph.kind == PH_T ? (s >= 0 && s <= A.nsteps) : (s >= 0 && s < A.nsteps);
-            s_item[slot][0] = s; s_item[slot][1] = lo; s_item[slot][2] = off - ph.first;
-            if (!live) state = 2;                                       // ticket of a phase outside the march: no work
-            else if (A.ticket) {
-                unsigned need; const unsigned* w = dependency(ph, s, need);
-                if (w && w != dep_ok) { if (ld_acquire(w) < need) ready = 0; else dep_ok = w; }
+    if (tid >= NT) {
+        // ================= scheduler warp: one thread draws tickets, resolves dependencies, signals completions =================
+        if (tid != NT) return;
+        // the completion counter an item of (phase, step) waits for, and the count it needs
+        auto dependency = [&](const Phase& ph, int s, unsigned& need) -> const unsigned* {
+            const int b = ph.prop_off & 1;
+            const unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
+            need = 0;
+            if (ph.kind == PH_T) { if (s <= 0) return nullptr; need = (unsigned)(A.nchunks * A.nY2); return cnt - C2 + 1; }
+            if (ph.kind == PH_Y1) { need = (unsigned)A.ntT; return cnt; }
+            if (ph.kind == PH_Z) { need = (unsigned)A.nY1; return cnt + 2 + ph.chunk; }
+            need = (unsigned)A.nZ; return cnt + 2 + A.nchunks + ph.chunk;
+        };
+        unsigned issued = 0, completed = 0, spins = 0;
+        unsigned tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : blockIdx.x;       // drawn one item ahead
+        bool have = false, exhausted = false;
+        int ps = 0, plo = 0, pidx = 0;                 // the item waiting for its dependency
+        const unsigned* pw = nullptr; unsigned pneed = 0;
+        const unsigned* dep_ok = nullptr;              // a counter once seen complete stays complete
+        int lo = 0;
+        for (;;) {
+            bool progress = false;
+            if (completed < issued) {                  // oldest item in flight: have all compute threads issued its stores?
+                const int slot = completed % R;
+                if (mbar_test(&s_done[slot], (completed / R) & 1)) {
+                    if (A.ticket) {
+                        const Phase ph = s_ph[s_item[slot][1]];
+                        const int b = ph.prop_off & 1, s = s_item[slot][0];
+                        unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
+                        unsigned* c = ph.kind == PH_T ? cnt : ph.kind == PH_Y2 ? cnt + 1 : ph.kind == PH_Y1 ? cnt + 2 + ph.chunk : cnt + 2 + A.nchunks + ph.chunk;
+                        __threadfence();
+                        atomicAdd(c, 1u);
+                    }
+                    ++completed; progress = true;
+                }
             }
+            if (!exhausted && issued - completed < (unsigned)R) {
+                if (!have) {
+                    const unsigned tk = tk_pending;
+                    if (tk >= total) {                 // end of march: publish the sentinel
+                        const int slot = issued % R;
+                        s_item[slot][3] = 0;
+                        mbar_arrive(&s_full[slot]);
+                        exhausted = true;
+                        continue;
+                    }
+                    tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : total;
+                    const int round = A.round0 + (int)(tk / (unsigned)A.tickets_per_round), off = (int)(tk % (unsigned)A.tickets_per_round);
+                    if (s_ph[lo].first > off) lo = 0;                                  // new round: restart the phase scan
+                    while (lo + 1 < A.nphases && s_ph[lo + 1].first <= off) ++lo;
+                    const Phase ph = s_ph[lo];
+                    ps = round - ((ph.prop_off >> 1) & 1); plo = lo; pidx = off - ph.first;
+                    const bool live = ph.kind == PH_T ? (ps >= 0 && ps <= A.nsteps) : (ps >= 0 && ps < A.nsteps);
+                    if (!live) continue;               // ticket of a phase outside the march: no work
+                    pw = A.ticket ? dependency(ph, ps, pneed) : nullptr;
+                    have = true; spins = 0;
+                }
+                bool ok = !pw || pw == dep_ok;
+                if (!ok) {
+                    ok = ld_acquire(pw) >= pneed;
+                    if (!ok && ++spins > (1u << 22)) { atomicExch(A.err, 1); ok = true; }      // never hang the GPU: flag it and carry on
+                }
+                if (ok) {
+                    if (pw) dep_ok = pw;
+                    const int slot = issued % R;
+                    s_item[slot][0] = ps; s_item[slot][1] = plo; s_item[slot][2] = pidx; s_item[slot][3] = 1;
+                    mbar_arrive(&s_full[slot]);
+                    ++issued; have = false; progress = true;
+                }
+            }
+            if (exhausted && completed == issued) break;
+            if (!progress) __nanosleep(32);
         }
-        s_item[slot][3] = state; s_item[slot][4] = ready;
-    };
+        return;
+    }
+
+    // ================= compute warps =================
     // every thread: its coordinates inside the item published in s_item[slot]
     const int Ny = A.g[1], Nz = A.g[2];
     auto coords = [&](int slot, Coords<T>& c) {
@@ -246,174 +319,141 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::THREADS, MarchCfg<T, 
         return b == 0 ? (step >= A.jA ? 1 : 0) : (step < A.Ns - A.jA ? 1 : 0);
     };
 
-    int slot = 0, cur_dim = -1;
+    int cur_dim = -1;
     bool cur_pref = false;
-    if (tid == 0) fetch(0);
-    __syncthreads();
-
-    for (;;) {
-        const int state = ((const volatile int*)s_item[slot])[3];
-        if (state == 0) break;
-        // ---- look one item ahead; block on the current item's dependency only if it was not met when it was drawn ----
-        if (tid == 0) {
-            fetch(slot ^ 1);
-            if (state == 1 && s_item[slot][4] == 0 && A.ticket) {
-                const Phase ph = s_ph[s_item[slot][1]];
-                unsigned need; const unsigned* w = dependency(ph, s_item[slot][0], need);
-                unsigned spins = 0;
-                while (w && ld_acquire(w) < need) {
-                    __nanosleep(100);
-                    if (++spins > (1u << 23)) { atomicExch(A.err, 1); break; }       // never hang the GPU: flag it and carry on
-                }
-                dep_ok = w;
-            }
-        }
-        __syncthreads();
+    for (unsigned it = 0;; ++it) {
+        const int slot = it % R, nslot = (it + 1) % R;
+        if (!mbar_wait(&s_full[slot], (it / R) & 1)) { atomicExch(A.err, 1); break; }      // descriptor published, dependency met
+        if (((const volatile int*)s_item[slot])[3] == 0) break;
         bool nxt_pref = false;
-        // stage the next item's primary input into s_pre (only if its dependency is already met)
+        // stage the next item's primary input into s_pre if the scheduler has already released it (per-thread decision:
+        // the staging buffers are thread-private)
         auto stage_next = [&]() {
-            const volatile int* nx = s_item[slot ^ 1];
-            if (nx[3] == 1 && nx[4] != 0) {
-                Coords<T> n; coords(slot ^ 1, n);
+            if (mbar_test(&s_full[nslot], ((it + 1) / R) & 1) && ((const volatile int*)s_item[nslot])[3] == 1) {
+                Coords<T> n; coords(nslot, n);
                 if (!(n.kind == PH_T && n.s == 0)) { prefetch_tile(s_pre, primary_src(n), n); nxt_pref = true; }
             }
         };
 
-        if (state == 1) {
-            C v[EPT];
-            int kind, st = 0;
-            bool contig;
-            {   // ---- load phase ----
-                Coords<T> c; coords(slot, c);
-                kind = c.kind; contig = kind == PH_Z;
-                const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
-                if (dim != cur_dim) {
-                    for (int i = tid; i < N; i += NT) {
-                        s_tw[i] = static_cast<const C*>(A.tw[dim])[i];
-                        s_tab[i] = static_cast<const T*>(A.tab[dim][0])[i];
-                        s_tab[N + i] = static_cast<const T*>(A.tab[dim][1])[i];
-                    }
-                    cur_dim = dim;
-                    __syncthreads();
+        C v[EPT];
+        int kind, st = 0, job = 0;
+        bool contig;
+        {   // ---- load phase ----
+            Coords<T> c; coords(slot, c);
+            kind = c.kind; contig = kind == PH_Z; job = c.job;
+            const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
+            if (dim != cur_dim) {                                     // new tables, possibly a new exchange layout: everyone must be done with the old
+                bar_compute<NT>();
+                for (int i = tid; i < N; i += NT) {
+                    s_tw[i] = static_cast<const C*>(A.tw[dim])[i];
+                    s_tab[i] = static_cast<const T*>(A.tab[dim][0])[i];
+                    s_tab[N + i] = static_cast<const T*>(A.tab[dim][1])[i];
                 }
-                const bool finish = c.s > 0;
-                // secondary input e4 -> s_stash, needed after the first diffusion (T finish, Z)
-                const bool e4_staged = (kind == PH_T && finish) || kind == PH_Z;
-                if (e4_staged) prefetch_tile(s_stash, static_cast<const C*>(A.e4[species(c.b, kind == PH_T ? c.s - 1 : c.s)]), c);
-                if (!(kind == PH_T && !finish)) {                     // primary input: staged by the previous iteration, or loaded directly
-                    if (cur_pref) {
-                        if (e4_staged) cp_async_wait<1>(); else cp_async_wait<0>();
-#pragma unroll
-                        for (int r = 0; r < EPT; ++r) v[r] = s_pre[r * NT + tid];
-                    } else {
-                        const C* src = primary_src(c);
-#pragma unroll
-                        for (int r = 0; r < EPT; ++r) v[r] = c.active ? ldcg(src + c.base0 + r * c.estride) : mk<T>(0, 0);
-                    }
-                }
-                // s_pre is free again: T items stage F for the combine, the others stage the next item's primary input now
-                if (kind == PH_T) { if (finish) prefetch_tile(s_pre, static_cast<const C*>(A.F[c.b]), c); }
-                else stage_next();
+                cur_dim = dim;
+                bar_compute<NT>();
             }
-            // T item tail: from q_s in v, write the slice, then b = e4 q_s -> stash, a = e4 b -> v   (start of step s)
-            auto emit_q_and_start = [&](bool combine) {
-                Coords<T> c; coords(slot, c);
-                const bool start = c.s < A.nsteps;
-                const int sp_now = species(c.b, c.s), sp_prev = species(c.b, c.s - 1);
-                C* qs = static_cast<C*>(A.q[c.b]) + (long long)c.s * A.M;
-                const C* e4s = static_cast<const C*>(A.e4[sp_now]);
-                const bool reload = !combine || sp_now != sp_prev;
+            const bool finish = c.s > 0;
+            // secondary input e4 -> s_stash, needed after the first diffusion (T finish, Z)
+            const bool e4_staged = (kind == PH_T && finish) || kind == PH_Z;
+            if (e4_staged) prefetch_tile(s_stash, static_cast<const C*>(A.e4[species(c.b, kind == PH_T ? c.s - 1 : c.s)]), c);
+            if (!(kind == PH_T && !finish)) {                         // primary input: staged by the previous iteration, or loaded directly
+                if (cur_pref) {
+                    if (e4_staged) cp_async_wait<1>(); else cp_async_wait<0>();
 #pragma unroll
-                for (int r = 0; r < EPT; ++r) {
-                    const int i = c.base0 + r * c.estride;
-                    C e = mk<T>(0, 0);
-                    if (combine) {                                    // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
-                        e = s_stash[r * NT + tid];
-                        const C f = s_pre[r * NT + tid];
-                        const C h = v[r] * e;
-                        v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
-                    }
-                    if (c.active) stcg(qs + i, v[r]);                 // the slice store IS the step's output write
-                    if (start) {
-                        if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
-                        const C hb = v[r] * e;
-                        s_stash[r * NT + tid] = hb;
-                        v[r] = hb * e;
-                    }
-                }
-                return start;
-            };
-            auto store_tile = [&](int which) {                        // 0: F, 1: H of the item's propagator
-                Coords<T> c; coords(slot, c);
-                C* dst = static_cast<C*>(which ? A.H[c.b] : A.F[c.b]);
-                if (c.active) {
+                    for (int r = 0; r < EPT; ++r) v[r] = s_pre[r * NT + tid];
+                } else {
+                    const C* src = primary_src(c);
 #pragma unroll
-                    for (int r = 0; r < EPT; ++r) stcg(dst + c.base0 + r * c.estride, v[r]);
+                    for (int r = 0; r < EPT; ++r) v[r] = c.active ? ldcg(src + c.base0 + r * c.estride) : mk<T>(0, 0);
                 }
-                return c.job;
-            };
+            }
+            // s_pre is free again: T items stage F for the combine, the others stage the next item's primary input now
+            if (kind == PH_T) { if (finish) prefetch_tile(s_pre, static_cast<const C*>(A.F[c.b]), c); }
+            else stage_next();
+        }
+        // T item tail: from q_s in v, write the slice, then b = e4 q_s -> stash, a = e4 b -> v   (start of step s)
+        auto emit_q_and_start = [&](bool combine) {
+            Coords<T> c; coords(slot, c);
+            const bool start = c.s < A.nsteps;
+            const int sp_now = species(c.b, c.s), sp_prev = species(c.b, c.s - 1);
+            C* qs = static_cast<C*>(A.q[c.b]) + (long long)c.s * A.M;
+            const C* e4s = static_cast<const C*>(A.e4[sp_now]);
+            const bool reload = !combine || sp_now != sp_prev;
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) {
+                const int i = c.base0 + r * c.estride;
+                C e = mk<T>(0, 0);
+                if (combine) {                                        // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
+                    e = s_stash[r * NT + tid];
+                    const C f = s_pre[r * NT + tid];
+                    const C h = v[r] * e;
+                    v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
+                }
+                if (c.active) stcg(qs + i, v[r]);                     // the slice store IS the step's output write
+                if (start) {
+                    if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
+                    const C hb = v[r] * e;
+                    s_stash[r * NT + tid] = hb;
+                    v[r] = hb * e;
+                }
+            }
+            return start;
+        };
+        auto store_tile = [&](int which) {                            // 0: F, 1: H of the item's propagator
+            Coords<T> c; coords(slot, c);
+            C* dst = static_cast<C*>(which ? A.H[c.b] : A.F[c.b]);
+            if (c.active) {
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) stcg(dst + c.base0 + r * c.estride, v[r]);
+            }
+        };
 
-            int job = 0;
-            if (kind == PH_T) {
-                if (((const volatile int*)s_item[slot])[0] == 0) {    // q(x,0) = 1, q+(x,s=1) = 1
+        bool run = true;
+        if (kind == PH_T && ((const volatile int*)s_item[slot])[0] == 0) {      // q(x,0) = 1, q+(x,s=1) = 1
 #pragma unroll
-                    for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
-                    emit_q_and_start(false);
+            for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
+            run = emit_q_and_start(false);
+            stage_next();
+            st = 1;
+        }
+#pragma unroll 1
+        while (run) {
+            // thread position inside the transform, and the table: full step for the F branch, half step otherwise
+            const int t = contig ? tid % TPP : (tid / TZ) % TPP, p = contig ? tid / TPP : tid % TZ;
+            C* xs = contig ? s_x : s_x + (tid / (TZ * TPP)) * (N * TZ);
+            const bool full = kind == PH_T ? (st == 1) : (job == 0);
+            diffuse<T, N, EPT, NT, LS, LC>(v, t, p, contig, s_tw, full ? s_tab : s_tab + N, xs, s_x);
+            if (kind == PH_T) {
+                if (st == 0) {
+                    cp_async_wait<0>();                               // e4 and F tiles of this item
+                    run = emit_q_and_start(true);
                     stage_next();
                     st = 1;
-                }
-            } else {
-                Coords<T> c; coords(slot, c);
-                job = c.job;
-            }
-#pragma unroll 1
-            for (;;) {
-                // thread position inside the transform, and the table: full step for the F branch, half step otherwise
-                const int t = contig ? tid % TPP : (tid / TZ) % TPP, p = contig ? tid / TPP : tid % TZ;
-                C* xs = contig ? s_x : s_x + (tid / (TZ * TPP)) * (N * TZ);
-                const bool full = kind == PH_T ? (st == 1) : (job == 0);
-                diffuse<T, N, EPT, LS, LC>(v, t, p, contig, s_tw, full ? s_tab : s_tab + N, xs, s_x);
-                if (kind == PH_T) {
-                    if (st == 0) {
-                        cp_async_wait<0>();                           // e4 and F tiles of this item
-                        const bool start = emit_q_and_start(true);
-                        stage_next();
-                        if (!start) break;
-                        st = 1;
-                    } else if (st == 1) {
-                        store_tile(0);
+                } else if (st == 1) {
+                    store_tile(0);
 #pragma unroll
-                        for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
-                        st = 2;
-                    } else {
-                        store_tile(1);
-                        break;
-                    }
-                } else if (kind == PH_Z && st == 0) {                 // F = e2 Dz F;  H = Dz'[e2 Dz' H]
-                    if (nxt_pref) cp_async_wait<1>(); else cp_async_wait<0>();      // the e4 tile (committed before the next item's tile)
-#pragma unroll
-                    for (int r = 0; r < EPT; ++r) {
-                        const C e = s_stash[r * NT + tid];
-                        v[r] = v[r] * (e * e);
-                    }
-                    if (job == 0) { store_tile(0); break; }
-                    st = 1;
-                } else {                                              // Y1, Y2, second z diffusion of H
-                    store_tile(job);
-                    break;
+                    for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
+                    st = 2;
+                } else {
+                    store_tile(1);
+                    run = false;
                 }
+            } else if (kind == PH_Z && st == 0) {                     // F = e2 Dz F;  H = Dz'[e2 Dz' H]
+                if (nxt_pref) cp_async_wait<1>(); else cp_async_wait<0>();      // the e4 tile (committed before the next item's tile)
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) {
+                    const C e = s_stash[r * NT + tid];
+                    v[r] = v[r] * (e * e);
+                }
+                if (job == 0) { store_tile(0); run = false; }
+                st = 1;
+            } else {                                                  // Y1, Y2, second z diffusion of H
+                store_tile(job);
+                run = false;
             }
         }
-        __syncthreads();                      // all stores of the item are issued
-        if (tid == 0 && state == 1 && A.ticket) {
-            const Phase ph = s_ph[s_item[slot][1]];
-            const int b = ph.prop_off & 1, s = s_item[slot][0];
-            unsigned* cnt = A.done + ((size_t)b * (A.Ns + 1) + s) * C2;
-            unsigned* c = ph.kind == PH_T ? cnt : ph.kind == PH_Y2 ? cnt + 1 : ph.kind == PH_Y1 ? cnt + 2 + ph.chunk : cnt + 2 + A.nchunks + ph.chunk;
-            __threadfence();
-            atomicAdd(c, 1u);
-        }
-        cur_pref = nxt_pref; slot ^= 1;
+        mbar_arrive(&s_done[slot]);                                   // this thread's stores of the item are issued
+        cur_pref = nxt_pref;
     }
     cp_async_wait<0>();
 }
