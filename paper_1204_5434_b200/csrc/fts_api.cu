@@ -215,13 +215,15 @@ static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool quer
     return cudaErrorInvalidValue;
 }
 // tz: pencils per strided tile = complex elements per 128-byte row, or 8 when Nz is shorter than that (complex64, Nz = 8)
+template <class T> static int tz_used(const Ctx* c) {
+    if (std::getenv("FTS_TZ8")) return 8;
+    return c->g[2] >= tz_of<T>() ? tz_of<T>() : 8;
+}
 template <class T>
 static cudaError_t launch_march(const Ctx* c, int N, const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
-    constexpr int TZ = tz_of<T>();
-    if (c->g[2] >= TZ) return launch_march_n<T, TZ>(N, A, grid, query, info, occ, st);
+    if (tz_used<T>(c) == tz_of<T>()) return launch_march_n<T, tz_of<T>()>(N, A, grid, query, info, occ, st);
     return launch_march_n<T, 8>(N, A, grid, query, info, occ, st);
 }
-template <class T> static int tz_used(const Ctx* c) { return c->g[2] >= tz_of<T>() ? tz_of<T>() : 8; }
 
 static int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
@@ -282,7 +284,7 @@ static fts_status plan_march(Ctx* c) {
     c->persistent = (Nx == Ny && Ny == Nz) && !(mode && std::strcmp(mode, "launch") == 0);
     // slab size: F and H of both propagators of `lag`-many slabs in flight must sit in L2 next to the streaming traffic
     const size_t plane = (size_t)Ny * Nz * c->esz;
-    size_t target = (size_t)4 << 20;
+    size_t target = (size_t)16 << 20;
     if (const char* e = std::getenv("FTS_SLAB_BYTES")) target = (size_t)std::atoll(e);
     int planes = Nx;
     while (planes > 1 && (size_t)planes * plane > target) planes >>= 1;

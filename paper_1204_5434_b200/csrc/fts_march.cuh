@@ -68,11 +68,13 @@ template <class T> __device__ __forceinline__ void stcg(cplx<T>* p, cplx<T> v) {
     typename vec2<T>::type w; w.x = v.x; w.y = v.y;
     __stcg(reinterpret_cast<typename vec2<T>::type*>(p), w);
 }
-__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+// Polling uses relaxed loads; the acquire fence (which invalidates L1) is paid once, when the counter is complete.
+__device__ __forceinline__ unsigned ld_relaxed(const unsigned* p) {
     unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void fence_acquire() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 
 template <class T, int N, int EPT, int TZ>
 struct MarchCfg {
@@ -252,8 +254,9 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
                 }
                 bool ok = !pw || pw == dep_ok;
                 if (!ok) {
-                    ok = ld_acquire(pw) >= pneed;
+                    ok = ld_relaxed(pw) >= pneed;
                     if (!ok && ++spins > (1u << 22)) { atomicExch(A.err, 1); ok = true; }      // never hang the GPU: flag it and carry on
+                    if (ok) fence_acquire();
                 }
                 if (ok) {
                     if (pw) dep_ok = pw;
@@ -342,7 +345,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
             Coords<T> c; coords(slot, c);
             kind = c.kind; contig = kind == PH_Z; job = c.job;
             const int dim = kind == PH_T ? 0 : (kind == PH_Z ? 2 : 1);
-            if (dim != cur_dim) {                                     // new tables, possibly a new exchange layout: everyone must be done with the old
+            if (dim != cur_dim) {                      // new tables, possibly a new exchange layout: everyone must be done with the old
                 bar_compute<NT>();
                 for (int i = tid; i < N; i += NT) {
                     s_tw[i] = static_cast<const C*>(A.tw[dim])[i];

@@ -139,7 +139,7 @@ struct Pencil {
         static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, -1>(v); });
         if constexpr (!S::ONE) {
             static_for<0, EPT>([&](auto rr) {
-                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                constexpr int r = decltype(rr)::value, k1 = r / S::G1;
                 if constexpr (k1 > 0) {
                     TW w = tw[r * S::TPP + t];
                     v[r] = v[r] * mk<T>((T)w.x, (T)w.y);
@@ -192,7 +192,7 @@ struct Pencil {
     static FTS_HD void inv_a(C (&v)[EPT], int t, const TW* tw) {
         if constexpr (!S::ONE) {
             static_for<0, EPT>([&](auto rr) {
-                constexpr int r = decltype(rr)::value, g = r % S::G1, k1 = r / S::G1;
+                constexpr int r = decltype(rr)::value, k1 = r / S::G1;
                 if constexpr (k1 > 0) {
                     TW w = tw[r * S::TPP + t];
                     v[r] = v[r] * mk<T>((T)w.x, -(T)w.y);
