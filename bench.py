@@ -232,7 +232,7 @@ def run_gpu(args):
     ms_e2e = timed(e2e_step, args.steps, 1)
     barrier()
 
-    # the march alone (fts_propagate: Boltzmann factors + all RQM4 passes + Q), for the roofline of the pass kernel
+    # the march alone (fts_propagate: Boltzmann factors + the persistent march kernel + Q), for the roofline of march_kernel
     g.set_fields(*devf)
     g.propagate()
     barrier()
@@ -268,7 +268,7 @@ def run_gpu(args):
     f_alg, b_alg = 30.0 * M * math.log2(M), 3.0 * E * M        # per RQM4 step of one propagator
     t_fp, t_hbm = f_alg / (best * 1e12), b_alg / (pk["hbm_gbs"] * 1e9)
     t_step = ms_march * 1e-3 / rq
-    pass_launches = 5 * cfg.Ns                                 # five fused pass launches per contour step (q and q+ batched)
+    pass_launches = 1                                          # the whole march of one solve is ONE persistent launch (cubic grids)
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
@@ -278,7 +278,7 @@ def run_gpu(args):
                 "peak_kind": f"vector {prec} FMA chains measured in this run (nominal {FP64_NOMINAL_TFLOPS if prec == 'f64' else FP32_NOMINAL_TFLOPS:.1f})"}
     else:
         roof = {"bound": "hbm", "achieved": b_alg / t_step / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": t_hbm / t_step, "peak_kind": pk_kind}
-    roof.update({"traffic": traffic, "kernel": "pass_kernel (all instantiations of the fused 1-D pass)", "launches_per_march": pass_launches,
+    roof.update({"traffic": traffic, "kernel": "march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve)", "launches_per_march": pass_launches,
                  "avg_launch_us": ms_march * 1e3 / pass_launches, "alg_flops_per_launch": f_alg * rq / pass_launches,
                  "alg_bytes_per_launch": b_alg * rq / pass_launches, "march_ms": ms_march, "march_launches_all_kernels": march_launches,
                  "hbm_view": {"achieved_GBs_algorithmic": b_alg / t_step / 1e9, "peak_GBs": pk["hbm_gbs"], "peak_kind": pk_kind,

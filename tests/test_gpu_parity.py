@@ -200,3 +200,69 @@ def test_determinism(B):
         Q, pa, pb = g.density_operators()
         outs.append((Q, pa.clone(), pb.clone()))
     assert outs[0][0] == outs[1][0] and torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])
+
+
+# ------------------------------------------------------------------------------------------------
+# the march schedules (persistent ticket kernel with L2 slabs, stream-ordered launches) and full-size runs
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("env", [{}, {"FTS_MARCH": "launch"}, {"FTS_SLAB_BYTES": "65536"}, {"FTS_SLAB_BYTES": "32768", "FTS_LAG": "3"}])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_march_schedules_agree(B, oracle, env, precision, monkeypatch):
+    """Cubic 32^3 grid (the persistent kernel's domain): one slab, 8 and 16 slabs with different pipeline lags, and the
+    one-launch-per-phase mode all reproduce the oracle; in fp64 they are also bit-identical to each other."""
+    for k in ("FTS_MARCH", "FTS_SLAB_BYTES", "FTS_LAG", "FTS_TZ8"):
+        monkeypatch.delenv(k, raising=False)
+    cfg = inputs.small_diblock(grid=(32, 32, 32), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
+    ref, _ = _pair(B, oracle, cfg, precision=precision)
+    ref.propagate()
+    Qr, par, pbr = ref.density_operators()
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)                      # read by fts_create
+    g, o = _pair(B, oracle, cfg, precision=precision)
+    g.propagate(); o.propagate()
+    Qg, pa, pb = g.density_operators()
+    Qo, oa, ob = o.density_operators()
+    tol = (1e-11, 1e-9) if precision == "f64" else (2e-4, 2e-4)
+    assert abs(Qg - Qo) <= tol[0] * abs(Qo)
+    assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tol[1] and np.max(np.abs(pb.cpu().numpy() - ob)) <= tol[1]
+    assert Qg == Qr and torch.equal(pa, par) and torch.equal(pb, pbr)      # the schedule does not change the arithmetic
+
+
+@pytest.mark.parametrize("model", ["edwards", "external"])
+def test_single_propagator_cubic_64(B, oracle, model):
+    """One propagator (q+ = q) through the persistent kernel at 64^3: T and U phases alternate with no second propagator."""
+    if model == "edwards":
+        cfg = inputs.config4(Ns=10)
+    else:
+        cfg = inputs.config1(grid=(64, 64, 64), cell=(8.0, 8.0, 8.0), Ns=10)
+    g, o = _pair(B, oracle, cfg)
+    _cmp_solve(g, o, 1e-11, 1e-9, False)
+    assert np.max(np.abs(g.get_slice(0, cfg.Ns).cpu().numpy() - o.get_slice(0, cfg.Ns))) < 1e-9
+
+
+@pytest.mark.parametrize("n,nsteps", [(128, 2), (256, 2)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_full_size_config5(B, oracle, n, nsteps, precision):
+    """BASELINE config 5 (256^3) and its 128^3 scaling point in the launch configuration bench.py times: oracle parity on
+    a truncated march (the oracle needs ~10 s per 256^3 step), then properties that hold at any size on the full march."""
+    cfg = inputs.config5(n)
+    dt = torch.complex128 if precision == "f64" else torch.complex64
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
+    g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
+    g.propagate(nsteps)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
+    o.set_fields(cfg.f0, cfg.f1)
+    o.propagate(nsteps)
+    tol = 1e-10 if precision == "f64" else 2e-4
+    for which in (0, 1):
+        ref = o.get_slice(which, nsteps)
+        assert np.max(np.abs(g.get_slice(which, nsteps).cpu().numpy() - ref)) <= tol * max(1.0, np.max(np.abs(ref))), which
+    del o
+    g.propagate()
+    Q, pa, pb = g.density_operators()
+    rel = 1e-11 if precision == "f64" else 2e-4
+    for j in (0, 1, 37, 50, 99, 100):
+        Qj = complex((g.get_slice(0, j).to(torch.complex128) * g.get_slice(1, cfg.Ns - j).to(torch.complex128)).mean().item())
+        assert abs(Qj - Q) <= rel * abs(Q), j
+    assert abs(complex(pa.to(torch.complex128).mean().item()) - cfg.fA) <= rel
+    assert abs(complex((pa + pb).to(torch.complex128).mean().item()) - 1.0) <= rel
