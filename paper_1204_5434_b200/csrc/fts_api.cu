@@ -215,9 +215,13 @@ static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool quer
     return cudaErrorInvalidValue;
 }
 // tz: pencils per strided tile = complex elements per 128-byte row, or 8 when Nz is shorter than that (complex64, Nz = 8)
+// Pencils per strided tile: one 128-byte row (8 complex128, 16 complex64) unless z is shorter.  complex64 at pencil
+// length 256 uses 64-byte rows instead: its 128-byte-row CTA (256 + 32 threads) is register-starved (measured: 681 vs 736 us per step at 256^3).
 template <class T> static int tz_used(const Ctx* c) {
+    const int full = tz_of<T>();
     if (std::getenv("FTS_TZ8")) return 8;
-    return c->g[2] >= tz_of<T>() ? tz_of<T>() : 8;
+    if (sizeof(T) == 4 && (c->g[0] >= 256 || c->g[1] >= 256 || c->g[2] >= 256)) return 8;
+    return c->g[2] >= full ? full : 8;
 }
 template <class T>
 static cudaError_t launch_march(const Ctx* c, int N, const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
