@@ -288,6 +288,8 @@ def run_gpu(args):
            "config": {"workload": cfg.name, "model": None, "grid": list(cfg.grid), "Ns": cfg.Ns, "kind": kind, "precision": prec,
                       "rqm4_steps_per_step": rqm4_steps_per_step(cfg, kind), "l2": "flushed between timed steps (256 MiB write)",
                       "parallelism": f"replicas x{world}" if world > 1 else "1 GPU"},
+           "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
+                                                                                      "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),
            "e2e": {"value": world * units * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": sum(h.numel() * h.element_size() for h in host),
                    "d2h_bytes_per_step": sum(b.numel() * b.element_size() for b in back[:1 if kind == 'propagate' else None])},
