@@ -155,6 +155,23 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def max_over_ranks(values, device, world):
+    """Device times of one replica per rank -> the slowest rank's (the job is as slow as its slowest replica).
+    Replicas share nothing on the data path, so this is the only collective of the bench."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
+def replica_seed(rank):
+    """Each replica is an independent CL run: its own Philox key."""
+    return 1000 + rank
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -178,7 +195,7 @@ def run_gpu(args):
     devf = [h.to(dev) for h in host]
     back = [torch.empty_like(h).pin_memory() for h in host]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)           # > 126 MB L2
-    seed = 1000 + rank
+    seed = replica_seed(rank)
 
     def step(i):
         if kind == "cl":
@@ -252,10 +269,7 @@ def run_gpu(args):
         torch.cuda.synchronize()
         best = max(best, 2.0 * nf / (a.elapsed_time(b) * 1e-3) / 1e12)
 
-    if world > 1:
-        t = torch.tensor([ms, ms_e2e, ms_march], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_e2e, ms_march = (float(x) for x in t.tolist())
+    ms, ms_e2e, ms_march = max_over_ranks([ms, ms_e2e, ms_march], dev, world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
