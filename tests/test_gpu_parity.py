@@ -205,12 +205,13 @@ def test_determinism(B):
 # ------------------------------------------------------------------------------------------------
 # the march schedules (persistent ticket kernel with L2 slabs, stream-ordered launches) and full-size runs
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("env", [{}, {"FTS_MARCH": "launch"}, {"FTS_SLAB_BYTES": "65536"}, {"FTS_SLAB_BYTES": "32768", "FTS_LAG": "3"}])
+@pytest.mark.parametrize("env", [{}, {"FTS_MARCH": "launch"}, {"FTS_SLAB_BYTES": "65536"}, {"FTS_SLAB_BYTES": "32768", "FTS_LAG": "3"},
+                                 {"FTS_INTERLEAVE": "0", "FTS_SLAB_BYTES": "131072"}, {"FTS_TZ8": "1"}])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_march_schedules_agree(B, oracle, env, precision, monkeypatch):
     """Cubic 32^3 grid (the persistent kernel's domain): one slab, 8 and 16 slabs with different pipeline lags, and the
     one-launch-per-phase mode all reproduce the oracle; in fp64 they are also bit-identical to each other."""
-    for k in ("FTS_MARCH", "FTS_SLAB_BYTES", "FTS_LAG", "FTS_TZ8"):
+    for k in ("FTS_MARCH", "FTS_SLAB_BYTES", "FTS_LAG", "FTS_TZ8", "FTS_INTERLEAVE", "FTS_EXTRA_SMEM"):
         monkeypatch.delenv(k, raising=False)
     cfg = inputs.small_diblock(grid=(32, 32, 32), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
     ref, _ = _pair(B, oracle, cfg, precision=precision)
@@ -226,6 +227,21 @@ def test_march_schedules_agree(B, oracle, env, precision, monkeypatch):
     assert abs(Qg - Qo) <= tol[0] * abs(Qo)
     assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tol[1] and np.max(np.abs(pb.cpu().numpy() - ob)) <= tol[1]
     assert Qg == Qr and torch.equal(pa, par) and torch.equal(pb, pbr)      # the schedule does not change the arithmetic
+
+
+def test_zero_and_one_step_march(B, oracle):
+    """Degenerate marches: 0 steps leaves q_0 = q+_0 = 1 and Q = 1; 1 step equals one Eq. 12 application of the oracle."""
+    cfg = inputs.small_diblock(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
+    g, o = _pair(B, oracle, cfg)
+    g.propagate(0)
+    for which in (0, 1):
+        assert torch.equal(g.get_slice(which, 0), torch.ones(cfg.grid, dtype=torch.complex128, device="cuda:0"))
+    g.propagate(1); o.propagate(1)
+    for which in (0, 1):
+        assert np.max(np.abs(g.get_slice(which, 1).cpu().numpy() - o.get_slice(which, 1))) < 1e-12
+    with pytest.raises(B.FtsError) as e:
+        g.density_operators()                          # a truncated march has no densities
+    assert e.value.status == 2
 
 
 @pytest.mark.parametrize("model", ["edwards", "external"])
