@@ -282,3 +282,67 @@ def test_full_size_config5(B, oracle, n, nsteps, precision):
         assert abs(Qj - Q) <= rel * abs(Q), j
     assert abs(complex(pa.to(torch.complex128).mean().item()) - cfg.fA) <= rel
     assert abs(complex((pa + pb).to(torch.complex128).mean().item()) - 1.0) <= rel
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE configs 2-4 at full size: trajectory parity over the first iterations, then spot parity — the oracle
+# solves once at the fields the GPU reached after many iterations (long runs are too slow for the oracle)
+# ------------------------------------------------------------------------------------------------
+def _spot(B, oracle, cfg, g, tolQ=1e-11, tolphi=1e-9):
+    a, b = g.get_fields()
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
+    o.set_fields(a.cpu().numpy().astype(np.complex128), None if b is None else b.cpu().numpy().astype(np.complex128))
+    g.propagate(); o.propagate()
+    Qg, pa, pb = g.density_operators()
+    Qo, oa, ob = o.density_operators()
+    assert np.isfinite(Qg.real) and abs(Qg - Qo) <= tolQ * abs(Qo), (Qg, Qo)
+    assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tolphi
+    if ob is not None:
+        assert np.max(np.abs(pb.cpu().numpy() - ob)) <= tolphi
+    return Qg, o
+
+
+def test_config2_scft_full_size(B, oracle):
+    """32^3, Ns = 100, fA = 0.3, chiN = 20, Seidel: 4 iterations side by side, then spot parity after 200 iterations."""
+    cfg = inputs.config2()
+    g, o = _pair(B, oracle, cfg)
+    for it in range(4):
+        Hg, rg = g.scft_step(*cfg.dt_scft, 1)
+        Ho, ro = o.scft_step(*cfg.dt_scft, 1)
+        assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9, it
+    res = []
+    for it in range(4, cfg.iters):
+        H, r = g.scft_step(*cfg.dt_scft, 1)
+        res.append(max(r))
+    assert res[-1] < res[0]                            # the relaxation makes progress
+    _spot(B, oracle, cfg, g)
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_config3_scft_spot_parity(B, oracle, precision):
+    """64^3, Ns = 200 (jA = 70), q+ batched with q: 30 Seidel iterations on the GPU, then one oracle solve at the final fields."""
+    cfg = inputs.config3()
+    g, _ = _pair(B, oracle, cfg, precision=precision)
+    for it in range(30):
+        H, r = g.scft_step(*cfg.dt_scft, 1)
+    assert np.isfinite(H.real) and max(r) < 1.0
+    if precision == "f64":
+        _spot(B, oracle, cfg, g)
+    else:
+        _spot(B, oracle, cfg, g, tolQ=2e-4, tolphi=2e-4)
+
+
+def test_config4_edwards_cl_full_size(B, oracle):
+    """64^3 Edwards solution, B = 1, C = 10, dt = 0.01: 2 CL steps side by side (identical Philox noise), spot parity of Q, phi and the
+    operators H, mu, Pi after 100 more steps."""
+    cfg = inputs.config4()
+    g, o = _pair(B, oracle, cfg)
+    for step in range(2):
+        g.cl_step(cfg.dt, 0, 4242, step); o.cl_step(cfg.dt, 0, 4242, step)
+    a, _ = g.get_fields(); oa, _ = o.get_fields()
+    assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-9
+    for step in range(2, 102):
+        g.cl_step(cfg.dt, 0, 4242, step)
+    _, o2 = _spot(B, oracle, cfg, g)
+    for x, y in zip(g.operators(), o2.operators()):    # H (Eq. 2), mu = ln C - ln Q, Pi (reading A-14) at the state reached
+        assert abs(x - y) < 1e-9 * max(1.0, abs(y))
