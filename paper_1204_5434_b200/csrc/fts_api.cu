@@ -139,7 +139,7 @@ template <class T> constexpr int tz_of() { return 128 / (2 * (int)sizeof(T)); } 
 template <class T>
 static cudaError_t launch_pass(const Ctx* c, int dim, PassArgs A, int njobs, cudaStream_t st) {
     const int Nx = c->g[0], Ny = c->g[1], Nz = c->g[2];
-    A.tab[0] = c->dim[dim].tab[0]; A.tab[1] = c->dim[dim].tab[1]; A.tw = c->dim[dim].tw;
+    A.tw = c->dim[dim].tw;
     A.k2x = c->dim[0].k2; A.k2y = c->dim[1].k2; A.k2z = c->dim[2].k2; A.Nz = Nz;
     A.invN = 1.0 / (double)c->g[dim];
     if (dim == 2) {
@@ -154,11 +154,7 @@ static cudaError_t launch_pass(const Ctx* c, int dim, PassArgs A, int njobs, cud
     return launch_pass_n<T, 8>(c->g[dim], A, njobs, st);
 }
 
-static Job mkjob(const void* in, void* out, int op, int pre = PRE_NONE, int tabA = 0, const void* e4 = nullptr, int second = 0, int tabB = 0,
-                 int post = POST_NONE, const void* aux = nullptr) {
-    Job j; j.in = in; j.out = out; j.e4 = e4; j.aux = aux; j.op = op; j.pre = pre; j.tabA = tabA; j.second = second; j.tabB = tabB; j.post = post;
-    return j;
-}
+static Job mkjob(const void* in, void* out, int op) { Job j; j.in = in; j.out = out; j.op = op; return j; }
 
 static int ew_blocks(size_t M) { size_t b = (M + 255) / 256; return (int)(b < 148 * 16 ? b : 148 * 16); }
 

@@ -1,9 +1,8 @@
 // fts_kernels.cuh — sm_100a kernels of the fts-b200 hot path.
 //
-// pass_kernel       one launch = one fused 1-D pass over up to four fields ("jobs"): load pencils into registers,
-//                   optional real-space Boltzmann multiply, [FFT -> spectral multiply -> IFFT] along the pencil with
-//                   one shared-memory exchange per transform, optional second diffusion (the z-pass of the half
-//                   branch), optional epilogue (Boltzmann multiply or the Richardson combine of PAPER.md:124 Eq. 12).
+// (The contour march itself is fts_march.cuh.)
+// pass_kernel       one launch = one 1-D pass of a 3-D transform over a field: forward, inverse, or — the x pass of the
+//                   field-update filters — forward, 3-D multiplier, inverse.  Used by the SCFT / Eq. 11 updates and Pi.
 // boltzmann_kernel  exp(-w ds/4) per species.
 // reduce_kernel     deterministic two-level sums / max (Q of Eq. 4, H of Eq. 2-3, residuals).
 // density_kernel    Simpson contour sums of q_j q+_{Ns-j} (Eq. 8).
@@ -18,24 +17,19 @@
 
 namespace fts {
 
-enum { OP_D = 0, OP_FWD = 1, OP_INV = 2, OP_FILT = 3 };
-enum { PRE_NONE = 0, PRE_E4 = 1, PRE_E2 = 2 };
-enum { POST_NONE = 0, POST_E2 = 1, POST_COMBINE = 2 };
+enum { OP_FWD = 1, OP_INV = 2, OP_FILT = 3 };
 enum { FILT_RATIONAL = 0, FILT_NEGK2 = 1 };
 
 struct Job {                  // block-uniform description of one field's trip through a pass
     const void* in;
     void* out;
-    const void* e4;           // exp(-w ds/4) of the species this step uses (e2 = e4*e4)
-    const void* aux;          // full-step branch, for POST_COMBINE
-    int op, pre, tabA, second, tabB, post;
+    int op;
 };
 
 struct Filt { int type; double a, b, c; };   // RATIONAL: a / (1 + b + c*g_D(k^2));  NEGK2: -a*k^2
 
 struct PassArgs {
     Job job[4];
-    const void* tab[2];       // real tables of this dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
     const void* tw;           // exp(-2 pi i m / N), m = 0..N-1
     int pstride;              // element stride along the pencil
     int outer_stride;         // strided passes: tile -> base offset = (tile / tiles_inner)*outer_stride + (tile % tiles_inner)*TZ
@@ -58,7 +52,7 @@ struct PassCfg {
     static constexpr int PS = CONTIG ? contig_ps<T, N, EPT>() : 1;
     static constexpr int XELEMS = S::ONE ? 0 : (CONTIG ? GPB * PS : GPB * N * TZ);   // one exchange buffer, in complex elements
     typedef typename std::conditional<CONTIG, XchgLayout<PS, S::R2 + 1, 1>, XchgLayout<1, S::R2 * (TZ ? TZ : 1), (TZ ? TZ : 1)>>::type L;
-    static constexpr size_t SMEM = (size_t)N * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T) + 2 * (size_t)XELEMS * sizeof(cplx<T>);
+    static constexpr size_t SMEM = (size_t)N * sizeof(cplx<T>) + 2 * (size_t)XELEMS * sizeof(cplx<T>);
 };
 
 __device__ __forceinline__ double debye_dev(double x) {          // g_D(x) = 2(e^-x + x - 1)/x^2
@@ -80,16 +74,11 @@ __global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(c
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* s_tw = reinterpret_cast<C*>(smem_raw);
-    T* s_tab = reinterpret_cast<T*>(s_tw + N);
-    C* s_x0 = reinterpret_cast<C*>(s_tab + 2 * N);
+    C* s_x0 = s_tw + N;
     C* s_x1 = s_x0 + Cfg::XELEMS;
 
     const int tid = threadIdx.x;
-    for (int i = tid; i < N; i += Cfg::THREADS) {
-        s_tw[i] = static_cast<const C*>(A.tw)[i];
-        s_tab[i] = static_cast<const T*>(A.tab[0])[i];
-        s_tab[N + i] = static_cast<const T*>(A.tab[1])[i];
-    }
+    for (int i = tid; i < N; i += Cfg::THREADS) s_tw[i] = static_cast<const C*>(A.tw)[i];
     __syncthreads();
 
     const Job J = A.job[blockIdx.y];
@@ -115,18 +104,9 @@ __global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(c
     }
 
     const C* in = static_cast<const C*>(J.in);
-    const C* e4 = static_cast<const C*>(J.e4);
     C v[EPT];
 #pragma unroll
     for (int r = 0; r < EPT; ++r) v[r] = active ? in[base + (t + TPP * r) * ps] : mk<T>(0, 0);
-    if (J.pre != PRE_NONE) {
-#pragma unroll
-        for (int r = 0; r < EPT; ++r) {
-            C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
-            if (J.pre == PRE_E2) e = e * e;
-            v[r] = v[r] * e;
-        }
-    }
 
     auto forward = [&]() {
         P::fwd_a(v, t, s_tw);
@@ -147,25 +127,7 @@ __global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(c
         P::inv_a(v, t, s_tw);
     };
 
-    if (J.op == OP_D) {
-        forward();
-        const T* tab = s_tab + J.tabA * N;
-#pragma unroll
-        for (int r = 0; r < EPT; ++r) v[r] = v[r] * tab[t + TPP * r];
-        inverse();
-        if (J.second) {       // z pass of the half branch: D_z^{1/2} e2 D_z^{1/2}
-#pragma unroll
-            for (int r = 0; r < EPT; ++r) {
-                C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
-                v[r] = v[r] * (e * e);
-            }
-            forward();
-            const T* tabb = s_tab + J.tabB * N;
-#pragma unroll
-            for (int r = 0; r < EPT; ++r) v[r] = v[r] * tabb[t + TPP * r];
-            inverse();
-        }
-    } else if (J.op == OP_FWD) {
+    if (J.op == OP_FWD) {
         forward();
     } else if (J.op == OP_INV) {
         const T s = (T)A.invN;
@@ -182,23 +144,6 @@ __global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(c
     }
 
     C* out = static_cast<C*>(J.out);
-    if (J.post == POST_E2) {
-#pragma unroll
-        for (int r = 0; r < EPT; ++r) {
-            C e = active ? e4[base + (t + TPP * r) * ps] : mk<T>(0, 0);
-            v[r] = v[r] * (e * e);
-        }
-    } else if (J.post == POST_COMBINE) {   // q' = (4 e4 half - full)/3   (Eq. 12)
-        const C* aux = static_cast<const C*>(J.aux);
-#pragma unroll
-        for (int r = 0; r < EPT; ++r) {
-            const int idx = base + (t + TPP * r) * ps;
-            C e = active ? e4[idx] : mk<T>(0, 0);
-            C f = active ? aux[idx] : mk<T>(0, 0);
-            C h = v[r] * e;
-            v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
-        }
-    }
     if (active) {
 #pragma unroll
         for (int r = 0; r < EPT; ++r) out[base + (t + TPP * r) * ps] = v[r];
@@ -208,11 +153,6 @@ __global__ void __launch_bounds__(PassCfg<T, N, EPT, TZ>::THREADS) pass_kernel(c
 // ------------------------------------------------------------------------------------------------
 // elementwise kernels
 // ------------------------------------------------------------------------------------------------
-template <class T>
-__global__ void fill_kernel(cplx<T>* a, int M, T re, T im) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) a[i] = mk<T>(re, im);
-}
-
 __device__ __forceinline__ cplx<double> cexp_d(cplx<double> z) {
     double s, c;
     sincos(z.y, &s, &c);
