@@ -34,6 +34,29 @@ template <class T> FTS_HD cplx<T> operator*(cplx<T> a, cplx<T> b) { return mk<T>
 template <class T> FTS_HD cplx<T> operator*(cplx<T> a, T s) { return mk<T>(a.x * s, a.y * s); }
 template <class T> FTS_HD cplx<T> conj(cplx<T> a) { return mk<T>(a.x, -a.y); }
 
+// complex64 on sm_100a: Blackwell's packed fp32 pair instructions (add/sub/mul/fma.f32x2 -> FADD2 / FMUL2 / FFMA2) do a
+// complex add in ONE instruction and a complex multiply in TWO (the (-y, x) swizzle is an operand modifier), which halves
+// the issue slots of the fp32 butterflies — the complex64 path is bound by instruction issue, not by the fp32 pipe.
+#if defined(__CUDA_ARCH__)
+__device__ __forceinline__ unsigned long long pk(float lo, float hi) { unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ cplx<float> unpk(unsigned long long r) { cplx<float> c; asm("mov.b64 {%0, %1}, %2;" : "=f"(c.x), "=f"(c.y) : "l"(r)); return c; }
+__device__ __forceinline__ cplx<float> operator+(cplx<float> a, cplx<float> b) {
+    unsigned long long r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a.x, a.y)), "l"(pk(b.x, b.y))); return unpk(r);
+}
+__device__ __forceinline__ cplx<float> operator-(cplx<float> a, cplx<float> b) {
+    unsigned long long r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a.x, a.y)), "l"(pk(b.x, b.y))); return unpk(r);
+}
+__device__ __forceinline__ cplx<float> operator*(cplx<float> a, cplx<float> b) {      // (ax bx - ay by, ay bx + ax by)
+    unsigned long long t, r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(pk(a.x, a.y)), "l"(pk(b.x, b.x)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk(-a.y, a.x)), "l"(pk(b.y, b.y)), "l"(t));
+    return unpk(r);
+}
+__device__ __forceinline__ cplx<float> operator*(cplx<float> a, float s) {
+    unsigned long long r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a.x, a.y)), "l"(pk(s, s))); return unpk(r);
+}
+#endif
+
 // cos(2 pi m / 16), m = 0..4, correctly rounded literals; everything else by symmetry.
 FTS_HD constexpr double cos16_q(int m) {
     return m == 0 ? 1.0 : m == 1 ? 0.92387953251128675613 : m == 2 ? 0.70710678118654752440 : m == 3 ? 0.38268343236508977173 : 0.0;
@@ -52,13 +75,14 @@ FTS_HD cplx<T> mul_w16(cplx<T> a) {
     else if constexpr (m == 4) return mk<T>(-a.y, a.x);      // * i
     else if constexpr (m == 8) return mk<T>(-a.x, -a.y);
     else if constexpr (m == 12) return mk<T>(a.y, -a.x);     // * -i
-    else if constexpr (m % 4 == 2) {                         // (+-1 +- i)/sqrt(2): 2 adds + 2 muls
+    else if constexpr (m % 4 == 2 && sizeof(T) == 4) {       // complex64: a packed complex multiply (2 instructions) is cheaper
+        return a * mk<T>((T)cos16(m), (T)sin16(m));
+    } else if constexpr (m % 4 == 2) {                       // (+-1 +- i)/sqrt(2): 2 adds + 2 muls
         constexpr T h = (T)0.70710678118654752440;
         constexpr T sc = (T)(cos16(m) > 0 ? 1 : -1), ss = (T)(sin16(m) > 0 ? 1 : -1);
         return mk<T>((sc * a.x - ss * a.y) * h, (ss * a.x + sc * a.y) * h);
     } else {
-        constexpr T c = (T)cos16(m), s = (T)sin16(m);
-        return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
+        return a * mk<T>((T)cos16(m), (T)sin16(m));
     }
 }
 
