@@ -217,6 +217,7 @@ static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool quer
 template <class T> static int tz_used(const Ctx* c) {
     const int full = tz_of<T>();
     if (std::getenv("FTS_TZ8")) return 8;
+    if (std::getenv("FTS_TZ16") && c->g[2] >= full) return full;
     if (sizeof(T) == 4 && (c->g[0] >= 256 || c->g[1] >= 256 || c->g[2] >= 256)) return 8;
     return c->g[2] >= full ? full : 8;
 }
