@@ -163,7 +163,8 @@ struct Coords {
     int base0, estride;                     // element offset of register r inside a field: base0 + r*estride   (M <= 2^24)
 };
 
-enum { MARCH_RING = 4 };      // item descriptors in flight between the scheduler warp and the compute warps
+enum { MARCH_RING = 4, MARCH_RING_F32 = 2 };      // item descriptors in flight between the scheduler warp and the compute warps
+                                                   // (A/B: complex64 with its 3 CTAs/SM balances better with fewer tickets held per CTA)
 
 template <class T, int N, int EPT, int TZ>
 __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N, EPT, TZ>::MINB) march_kernel(const MarchArgs A) {
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
     typedef cplx<T> C;
     constexpr int TPP = S::TPP;
     constexpr int NT = Cfg::THREADS;          // compute threads; warp NT/32 is the scheduler
-    constexpr int R = MARCH_RING;
+    constexpr int R = sizeof(T) == 4 ? MARCH_RING_F32 : MARCH_RING;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* s_tw = reinterpret_cast<C*>(smem_raw);
