@@ -346,3 +346,26 @@ def test_config4_edwards_cl_full_size(B, oracle):
     _, o2 = _spot(B, oracle, cfg, g)
     for x, y in zip(g.operators(), o2.operators()):    # H (Eq. 2), mu = ln C - ln Q, Pi (reading A-14) at the state reached
         assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+
+
+@pytest.mark.parametrize("model", ["diblock", "edwards"])
+def test_fp32_field_updates_track_the_fp64_oracle(B, oracle, model):
+    """complex64 mode through the update kernels: 5 CL steps (identical Philox noise, rounded to float) and, for the
+    diblock, 3 SCFT iterations stay within the fp32 tolerance of north_star (2e-4 relative) of the fp64 oracle."""
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4, C=20.0, complex_fields=False)
+    else:
+        cfg = inputs.config4(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10)
+    g, o = _pair(B, oracle, cfg, precision="f32")
+    for step in range(5):
+        g.cl_step(0.01, 0, 77, step); o.cl_step(0.01, 0, 77, step)
+    a, b = g.get_fields(); oa, ob = o.get_fields()
+    assert np.max(np.abs(a.cpu().numpy() - oa)) < 2e-4 * max(1.0, np.max(np.abs(oa)))
+    if model == "diblock":
+        assert np.max(np.abs(b.cpu().numpy() - ob)) < 2e-4 * max(1.0, np.max(np.abs(ob)))
+        cfg2 = inputs.config2(grid=(16, 16, 16), Ns=20)
+        g2, o2 = _pair(B, oracle, cfg2, precision="f32")
+        for it in range(3):
+            Hg, rg = g2.scft_step(5.0, 5.0, 1)
+            Ho, ro = o2.scft_step(5.0, 5.0, 1)
+            assert abs(Hg - Ho) < 2e-4 * max(1.0, abs(Ho)) and abs(rg[0] - ro[0]) < 2e-4 and abs(rg[1] - ro[1]) < 2e-4 * max(1.0, ro[1]), it
