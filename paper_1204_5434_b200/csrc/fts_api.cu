@@ -33,7 +33,7 @@ struct Ctx {
     Phase* phases;            // device: persistent template at [0], the four per-launch templates at [MARCH_MAXPH * (1..4)]
     unsigned* counters;       // device: completion counters, then ticket and error flag
     size_t counters_bytes;
-    int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms;
+    int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
     std::string err;
 };
 
@@ -335,9 +335,12 @@ static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
         A.phases = c->phases; A.nphases = c->nph; A.tickets_per_round = c->tickets_per_round; A.round0 = 0; A.round1 = nsteps;
         A.ntT = c->cnt[PH_T]; A.nY1 = c->cnt[PH_Y1]; A.nZ = c->cnt[PH_Z]; A.nY2 = c->cnt[PH_Y2];
         A.ticket = (unsigned*)((char*)c->counters + c->counters_bytes - 256);
-        int occ = 0; MarchInfo mi;
-        CK(launch_march<T>(c, c->g[0], A, 0, true, &mi, &occ, st));
-        if (occ < 1) { c->err = "march kernel does not fit on an SM"; return FTS_ECUDA; }
+        if (c->occ < 1) {                              // resident CTAs per SM of this instantiation, queried once per context
+            MarchInfo mi;
+            CK(launch_march<T>(c, c->g[0], A, 0, true, &mi, &c->occ, st));
+            if (c->occ < 1) { c->err = "march kernel does not fit on an SM"; return FTS_ECUDA; }
+        }
+        const int occ = c->occ;
         long long total = (long long)(nsteps + 1) * c->tickets_per_round;
         long long grid = (long long)occ * c->sms;
         if (grid > total) grid = total;
@@ -617,7 +620,7 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
         c->q[i] = c->ws + Lo.off_q[i]; c->phi[i] = c->ws + Lo.off_phi[i]; c->G[i] = c->ws + Lo.off_G[i];
     }
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
-    c->have_fields = c->have_prop = false; c->marched = 0;
+    c->have_fields = c->have_prop = false; c->marched = 0; c->occ = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
     if (!rc) rc = DISPATCH(plan_march<double>(c), plan_march<float>(c));
     if (rc) { delete c; return rc; }
