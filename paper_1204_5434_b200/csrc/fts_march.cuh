@@ -11,16 +11,17 @@
 // (D = exp(ds d^2/dx_d^2) applied as FFT -> real table -> IFFT along one dimension, D' the same at ds/2; the three
 // 1-D factors of exp(-k^2 ds) commute, so the half branch is ordered x y z | z y x and its two z diffusions meet
 // around the real-space multiply.)  F and H are updated in place.  Per step and propagator the items move
-// 6 (T) + 4 (Y1) + 5 (Z) + 2 (Y2) fields through L2; Y1, Z and Y2 are issued slab by slab over x-ranges small
-// enough that a slab of F and H stays resident in the 126 MB L2 from its Y1 read to its Y2 write, so HBM sees
-// about 11 field transfers per step instead of 17.
+// 6 (T) + 4 (Y1) + 5 (Z) + 2 (Y2) fields through L2.  Y1, Z and Y2 can be issued slab by slab over x-ranges small
+// enough that a slab of F and H stays resident in the 126 MB L2 from its Y1 read to its Y2 write (HBM then sees
+// about 11-13 field transfers per step instead of 17); the default is one slab, because the march is not HBM-bound
+// and coarser phases measure faster.
 //
-// Scheduling: work items are handed out in a fixed global order through an atomic ticket; an item waits (acquire
-// poll on a per-phase completion counter) for the phase it depends on, which always precedes it in ticket order, so
-// the kernel is deadlock-free for any grid size.  The q and q+ marches are independent; their phases are
-// interleaved half a step apart so that the whole-field dependency T <-> {Y1,Z,Y2} of one propagator is always
-// separated by a block of the other propagator's work.  Data crosses CTAs only through L2: every field access is
-// ld.global.cg / st.global.cg.
+// Scheduling: work items are handed out in a fixed global order through an atomic ticket, drawn by one scheduler warp
+// per CTA; an item is released to the compute warps (mbarrier ring) when the completion counter of the phase it
+// depends on is full.  That phase always precedes it in ticket order, so the kernel is deadlock-free for any grid
+// size.  The q and q+ marches are independent; their phases alternate and run half a step apart so that every
+// dependency is separated by work of the other propagator.  Data crosses CTAs only through L2: every field access is
+// ld.global.cg / st.global.cg / cp.async.
 #ifndef FTS_MARCH_CUH
 #define FTS_MARCH_CUH
 
