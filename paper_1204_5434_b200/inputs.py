@@ -113,3 +113,18 @@ def small_diblock(grid=(8, 16, 32), cell=(3.0, 4.0, 5.0), Ns=20, fA=0.4, chiN=12
 def random_complex_field(grid, seed, scale=0.3, mean=0.0):
     rng = _rng(50, seed)
     return mean + scale * (rng.normal(size=grid) + 1j * rng.normal(size=grid))
+
+
+def developed(cfg, seed=0):
+    """Seeded fields with the amplitude and roughness of a run that has left its initial condition (stronger
+    segregation, a non-zero pressure-like field, complex parts as in CL) — used to compare one solve at a
+    'late-time' state without feeding anything produced by the CUDA path to the oracle."""
+    rng = _rng(70, seed)
+    X = _coords(cfg.grid, cfg.cell)
+    smooth = sum(np.cos(2.0 * np.pi * (k + 1) * X[k] / cfg.cell[k]) for k in range(3))
+    if cfg.model == "diblock":
+        f1 = 2.0 * cfg.f1.real + rng.normal(0.0, 0.1, cfg.grid) + 1j * rng.normal(0.0, 0.05, cfg.grid)
+        f0 = 0.4 * smooth + rng.normal(0.0, 0.1, cfg.grid) + 1j * rng.normal(0.0, 0.05, cfg.grid)
+        return np.asarray(f0, np.complex128), np.asarray(f1, np.complex128)
+    f0 = cfg.f0 + 0.2 * smooth + rng.normal(0.0, 0.3, cfg.grid) + 1j * rng.normal(0.0, 0.2, cfg.grid)
+    return np.asarray(f0, np.complex128), None

@@ -285,13 +285,17 @@ def test_full_size_config5(B, oracle, n, nsteps, precision):
 
 
 # ------------------------------------------------------------------------------------------------
-# BASELINE configs 2-4 at full size: trajectory parity over the first iterations, then spot parity — the oracle
-# solves once at the fields the GPU reached after many iterations (long runs are too slow for the oracle)
+# BASELINE configs 2-4 at full size: trajectory parity over the first iterations; parity of one solve at seeded
+# "developed" fields (inputs.developed: nothing the CUDA path produced is ever fed to the oracle); and properties that
+# hold at any size after a long GPU run (the oracle is too slow for 200-1000 iterations)
 # ------------------------------------------------------------------------------------------------
-def _spot(B, oracle, cfg, g, tolQ=1e-11, tolphi=1e-9):
-    a, b = g.get_fields()
+def _developed_solve_parity(B, oracle, cfg, precision="f64", tolQ=1e-11, tolphi=1e-9, operators=False):
+    f0, f1 = inputs.developed(cfg)
+    dt = torch.complex128 if precision == "f64" else torch.complex64
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
-    o.set_fields(a.cpu().numpy().astype(np.complex128), None if b is None else b.cpu().numpy().astype(np.complex128))
+    g.set_fields(_dev(f0, dt), None if f1 is None else _dev(f1, dt))
+    o.set_fields(f0, f1)
     g.propagate(); o.propagate()
     Qg, pa, pb = g.density_operators()
     Qo, oa, ob = o.density_operators()
@@ -299,11 +303,28 @@ def _spot(B, oracle, cfg, g, tolQ=1e-11, tolphi=1e-9):
     assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tolphi
     if ob is not None:
         assert np.max(np.abs(pb.cpu().numpy() - ob)) <= tolphi
-    return Qg, o
+    if operators:
+        for x, y in zip(g.operators(), o.operators()):     # H (Eq. 2), mu = ln C - ln Q, Pi (reading A-14)
+            assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+
+
+def _invariants(g, cfg, rel):
+    g.propagate()
+    Q, pa, pb = g.density_operators()
+    assert np.isfinite(Q.real) and np.isfinite(Q.imag)
+    two = cfg.model == "diblock"
+    for j in (0, cfg.Ns // 3, cfg.Ns):
+        Qj = complex((g.get_slice(0, j).to(torch.complex128) * g.get_slice(1, cfg.Ns - j).to(torch.complex128)).mean().item())
+        assert abs(Qj - Q) <= rel * abs(Q), j
+    tot = pa + pb if two else pa
+    assert abs(complex(tot.to(torch.complex128).mean().item()) - 1.0) <= rel
+    if two:
+        assert abs(complex(pa.to(torch.complex128).mean().item()) - cfg.fA) <= rel
 
 
 def test_config2_scft_full_size(B, oracle):
-    """32^3, Ns = 100, fA = 0.3, chiN = 20, Seidel: 4 iterations side by side, then spot parity after 200 iterations."""
+    """32^3, Ns = 100, fA = 0.3, chiN = 20, Seidel: 4 iterations side by side with the oracle; all 200 iterations on the
+    GPU (residual falls, invariants hold); one solve at developed fields against the oracle."""
     cfg = inputs.config2()
     g, o = _pair(B, oracle, cfg)
     for it in range(4):
@@ -315,26 +336,29 @@ def test_config2_scft_full_size(B, oracle):
         H, r = g.scft_step(*cfg.dt_scft, 1)
         res.append(max(r))
     assert res[-1] < res[0]                            # the relaxation makes progress
-    _spot(B, oracle, cfg, g)
+    _invariants(g, cfg, 1e-11)
+    _developed_solve_parity(B, oracle, cfg)
 
 
 @pytest.mark.parametrize("precision", ["f64", "f32"])
-def test_config3_scft_spot_parity(B, oracle, precision):
-    """64^3, Ns = 200 (jA = 70), q+ batched with q: 30 Seidel iterations on the GPU, then one oracle solve at the final fields."""
+def test_config3_scft_full_size(B, oracle, precision):
+    """64^3, Ns = 200 (jA = 70), q+ batched with q: 30 Seidel iterations on the GPU (invariants), one solve at developed
+    fields against the oracle."""
     cfg = inputs.config3()
     g, _ = _pair(B, oracle, cfg, precision=precision)
     for it in range(30):
         H, r = g.scft_step(*cfg.dt_scft, 1)
     assert np.isfinite(H.real) and max(r) < 1.0
+    _invariants(g, cfg, 1e-11 if precision == "f64" else 2e-4)
     if precision == "f64":
-        _spot(B, oracle, cfg, g)
+        _developed_solve_parity(B, oracle, cfg)
     else:
-        _spot(B, oracle, cfg, g, tolQ=2e-4, tolphi=2e-4)
+        _developed_solve_parity(B, oracle, cfg, precision="f32", tolQ=2e-4, tolphi=2e-4)
 
 
 def test_config4_edwards_cl_full_size(B, oracle):
-    """64^3 Edwards solution, B = 1, C = 10, dt = 0.01: 2 CL steps side by side (identical Philox noise), spot parity of Q, phi and the
-    operators H, mu, Pi after 100 more steps."""
+    """64^3 Edwards solution, B = 1, C = 10, dt = 0.01: 2 CL steps side by side (identical Philox noise); 100 more steps on
+    the GPU (invariants); one solve plus the operators H, mu, Pi at developed fields against the oracle."""
     cfg = inputs.config4()
     g, o = _pair(B, oracle, cfg)
     for step in range(2):
@@ -343,9 +367,8 @@ def test_config4_edwards_cl_full_size(B, oracle):
     assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-9
     for step in range(2, 102):
         g.cl_step(cfg.dt, 0, 4242, step)
-    _, o2 = _spot(B, oracle, cfg, g)
-    for x, y in zip(g.operators(), o2.operators()):    # H (Eq. 2), mu = ln C - ln Q, Pi (reading A-14) at the state reached
-        assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+    _invariants(g, cfg, 1e-11)
+    _developed_solve_parity(B, oracle, cfg, operators=True)
 
 
 @pytest.mark.parametrize("model", ["diblock", "edwards"])
