@@ -392,3 +392,24 @@ def test_fp32_field_updates_track_the_fp64_oracle(B, oracle, model):
             Hg, rg = g2.scft_step(5.0, 5.0, 1)
             Ho, ro = o2.scft_step(5.0, 5.0, 1)
             assert abs(Hg - Ho) < 2e-4 * max(1.0, abs(Ho)) and abs(rg[0] - ro[0]) < 2e-4 and abs(rg[1] - ro[1]) < 2e-4 * max(1.0, ro[1]), it
+
+
+@pytest.mark.parametrize("n,precision,reps", [(16, "f64", 500), (32, "f64", 1000), (64, "f64", 300), (64, "f32", 300), (128, "f64", 60), (128, "f32", 60), (256, "f64", 6)])
+def test_march_soak_bit_identical(B, n, precision, reps):
+    """The dependency protocol under changing timing: repeated solves of the same fields (persistent kernel, work items
+    claimed dynamically by ~300-450 CTAs) must be bit-identical every time; a race would show as a differing bit."""
+    cfg = inputs.small_diblock(grid=(n, n, n), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
+    dt = torch.complex128 if precision == "f64" else torch.complex64
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", precision=precision, **_kw(cfg))
+    g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
+    g.propagate()
+    Q0, pa0, pb0 = g.density_operators()
+    pa0, pb0 = pa0.clone(), pb0.clone()
+    last = g.get_slice(1, cfg.Ns).clone()
+    for rep in range(reps):
+        if rep % 3 == 1:
+            torch.empty(64 << 20, dtype=torch.uint8, device="cuda:0").zero_()      # perturb L2 / timing
+        g.propagate()
+        Q, pa, pb = g.density_operators()
+        assert Q == Q0 and torch.equal(pa, pa0) and torch.equal(pb, pb0), rep
+        assert torch.equal(g.get_slice(1, cfg.Ns), last), rep
