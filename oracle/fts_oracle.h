@@ -17,7 +17,9 @@
  *
  * Pins (tests/test_oracle_pins.py): direct DFT, uniform-field closed form, dense 4^3 operator and
  * dense matrix exponential, 4th-order convergence, mean_x q_j q+_{Ns-j} = Q, Debye response,
- * homogeneous saddles, Philox known-answer vectors.  The Pi operator is "parity unpinned" beyond
+ * homogeneous saddles (diblock H, Edwards H/mu/Pi), Philox known-answer vectors; the SCFT multipliers and the
+ * Eq. 10-11 (scheme 1) update, both models, to the backward-Euler / IMEX step of the linearised dynamics and to
+ * exactly filtered noise at the saddle.  The Pi operator is "parity unpinned" beyond
  * a finite-difference dln Q/dV check and its mean-field value (derived, not printed in the paper).
  */
 #ifndef FTS_ORACLE_H

@@ -247,6 +247,141 @@ def test_edwards_noise_free_relaxation_reaches_saddle(oracle, scheme):
     assert abs(Pi - (Cc + Cc ** 2 / (2 * B))) < 1e-8
 
 
+def _block_debye(fA, k2):
+    """Textbook diblock Debye functions g_AA, g_BB, g_AB at x = k^2 Rg^2 (same forms as test_debye_response_diblock_blocks)."""
+    fB = 1.0 - fA
+    gAA = 2.0 * (np.exp(-fA * k2) + fA * k2 - 1.0) / k2 ** 2
+    gBB = 2.0 * (np.exp(-fB * k2) + fB * k2 - 1.0) / k2 ** 2
+    gAB = (1 - np.exp(-fA * k2)) * (1 - np.exp(-fB * k2)) / k2 ** 2
+    return gAA, gBB, gAB
+
+
+@pytest.mark.parametrize("n,dtp,dtm", [(1, 5.0, 5.0), (2, 0.7, 2.5), (3, 12.0, 0.3)])
+def test_scft_step_is_the_semi_implicit_step_of_the_linearised_dynamics(oracle, n, dtp, dtm):
+    """Pins the two multipliers of the SCFT update (reading A-10; Eq. 10-11 at zero noise).
+
+    Around the homogeneous state (fA = 1/2, W- = 0) a single mode eps*cos(kx) has the linear-response forces
+    F+ = -g_D(k^2) W+ and F- = (2/chiN - S(k^2)) W-, S = g_AA + g_BB - 2 g_AB.  Eq. 11 treats g_D (for
+    W+) and 2/chiN (for W-) implicitly, so ONE step must give the backward-Euler / IMEX amplitudes
+        W+' = W+ / (1 + dt+ g_D),      W-' = W- (1 + dt- S) / (1 + 2 dt-/chiN)
+    up to O(eps^2) and the O(ds^4) contour error.  A denominator 1 + dt+ or 1 + dt-*2 fails this at every (k, dt)."""
+    grid, cell, Ns, fA, chiN, eps = (16, 1, 1), (4.0, 1.0, 1.0), 64, 0.5, 12.0, 1e-5
+    x = np.arange(16) * (4.0 / 16)
+    c = np.cos(2 * np.pi * n * x / 4.0).reshape(grid)
+    k2 = (2 * np.pi * n / 4.0) ** 2
+    gAA, gBB, gAB = _block_debye(fA, k2)
+    o = oracle.Oracle(grid, cell, Ns, "diblock", fA=fA, chiN=chiN)
+    o.set_fields((eps * c).astype(np.complex128), np.zeros(grid, np.complex128))
+    o.scft_step(dtp, dtm, seidel=0)
+    a, b = o.get_fields()
+    amp = 2.0 * np.mean(a.real * c)
+    assert abs(amp / eps - 1.0 / (1.0 + dtp * _gD(k2))) < 2e-6
+    assert np.max(np.abs(a - amp * c)) < 1e-3 * eps and np.max(np.abs(b)) < 1e-3 * eps      # no other mode, W- untouched
+    o.set_fields(np.zeros(grid, np.complex128), (eps * c).astype(np.complex128))
+    o.scft_step(dtp, dtm, seidel=0)
+    a, b = o.get_fields()
+    amp = 2.0 * np.mean(b.real * c)
+    S = gAA + gBB - 2.0 * gAB
+    assert abs(amp / eps - (1.0 + dtm * S) / (1.0 + 2.0 * dtm / chiN)) < 2e-6
+    assert np.max(np.abs(b - amp * c)) < 1e-3 * eps and np.max(np.abs(a)) < 1e-3 * eps
+
+
+def _k2_grid(grid, cell):
+    ks = [2 * np.pi * np.fft.fftfreq(g, d=L / g) for g, L in zip(grid, cell)]
+    KX, KY, KZ = np.meshgrid(*ks, indexing="ij")
+    return KX ** 2 + KY ** 2 + KZ ** 2
+
+
+def _gD_safe(x):
+    x = np.asarray(x, float)
+    out = np.ones_like(x)
+    nz = x > 1e-8
+    out[nz] = 2.0 * (np.exp(-x[nz]) + x[nz] - 1.0) / x[nz] ** 2
+    return out
+
+
+@pytest.mark.parametrize("n,dt", [(1, 0.3), (3, 1.7)])
+def test_cl_scheme1_edwards_is_backward_euler_and_filters_the_noise(oracle, n, dt):
+    """Pins cl_step scheme=1, Edwards branch (reading A-11; Eq. 10-11).
+
+    (a) noise off, Omega = Omega* + eps cos(kx): the linearised force is (B + C g_D(k^2)) dOmega (chain feels i*Omega),
+        Eq. 10 treats exactly that operator implicitly, so one step gives dOmega' = dOmega / (1 + l dt (B + C g_D)).
+    (b) noise on, AT the saddle (force identically zero): solving Eq. 10 for the new field divides the noise by the same
+        operator, dOmega^(k) = eta^(k) / (1 + l dt (B + C g_D(k^2))), with eta = sqrt(2 l dt/dV) N(0,1) (the normals and
+        their amplitude are pinned separately above).  Undivided noise (Eq. 11 as printed) fails (b)."""
+    grid, cell, Ns, B, Cc, lam, eps = (16, 1, 1), (4.0, 1.0, 1.0), 64, 2.0, 3.0, 0.8, 1e-5
+    x = np.arange(16) * (4.0 / 16)
+    c = np.cos(2 * np.pi * n * x / 4.0).reshape(grid)
+    k2 = (2 * np.pi * n / 4.0) ** 2
+    o = oracle.Oracle(grid, cell, Ns, "edwards", B=B, Cc=Cc, lambda_plus=lam, noise_scale=0.0)
+    o.set_fields((-1j * Cc / B + eps * c).astype(np.complex128))
+    o.cl_step(dt, 1, 1, 0)
+    f, _ = o.get_fields()
+    amp = 2.0 * np.mean((f - (-1j * Cc / B)).real * c)
+    assert abs(amp / eps - 1.0 / (1.0 + lam * dt * (B + Cc * _gD(k2)))) < 2e-6
+    grid3, cell3 = (4, 8, 2), (3.0, 4.0, 5.0)
+    M = int(np.prod(grid3))
+    o = oracle.Oracle(grid3, cell3, 8, "edwards", B=B, Cc=Cc, lambda_plus=lam)
+    o.set_fields(np.full(grid3, -1j * Cc / B, np.complex128))
+    o.cl_step(dt, 1, 11, 5)
+    f, _ = o.get_fields()
+    eta = np.sqrt(2 * lam * dt / (np.prod(cell3) / M)) * np.array([oracle.normal(11, 5, 0, i) for i in range(M)]).reshape(grid3)
+    want = np.fft.ifftn(np.fft.fftn(eta) / (1.0 + lam * dt * (B + Cc * _gD_safe(_k2_grid(grid3, cell3)))))
+    assert np.max(np.abs((f - (-1j * Cc / B)) - want)) < 1e-12
+    assert np.max(np.abs((f - (-1j * Cc / B)) - eta)) > 1e-3                         # the filter is not a no-op here
+
+
+def test_cl_scheme1_diblock_is_backward_euler_and_filters_the_noise(oracle):
+    """Pins cl_step scheme=1, diblock branch (reading A-11): W+ implicit in C g_D(k^2), W- implicit in 2C/chiN.
+
+    (a) noise off, W+ = eps cos(kx) on the fA = 1/2 homogeneous state: F+ = -g_D W+, so W+' = W+/(1 + l+ dt C g_D);
+        W- = eps cos: W-' = W- (1 + l- dt C S)/(1 + 2 l- dt C/chiN), S = g_AA + g_BB - 2 g_AB.
+    (b) noise on at the homogeneous saddle W- = chiN(2fA-1)/2 (both forces vanish, test_diblock_homogeneous_saddle):
+        dW+ = i F^-1{eta+^/(1 + l+ dt C g_D)},  dW- = eta-/(1 + 2 l- dt C/chiN)."""
+    grid, cell, Ns, fA, chiN, Cc, lp, lm, dt, eps = (16, 1, 1), (4.0, 1.0, 1.0), 64, 0.5, 12.0, 4.0, 0.7, 1.3, 0.4, 1e-5
+    x = np.arange(16) * (4.0 / 16)
+    c = np.cos(2 * np.pi * 2 * x / 4.0).reshape(grid)
+    k2 = (2 * np.pi * 2 / 4.0) ** 2
+    gAA, gBB, gAB = _block_debye(fA, k2)
+    kw = dict(fA=fA, chiN=chiN, Cc=Cc, lambda_plus=lp, lambda_minus=lm)
+    o = oracle.Oracle(grid, cell, Ns, "diblock", noise_scale=0.0, **kw)
+    o.set_fields((eps * c).astype(np.complex128), np.zeros(grid, np.complex128))
+    o.cl_step(dt, 1, 1, 0)
+    a, _ = o.get_fields()
+    assert abs(2.0 * np.mean(a.real * c) / eps - 1.0 / (1.0 + lp * dt * Cc * _gD(k2))) < 2e-6
+    o.set_fields(np.zeros(grid, np.complex128), (eps * c).astype(np.complex128))
+    o.cl_step(dt, 1, 1, 0)
+    _, b = o.get_fields()
+    S = gAA + gBB - 2.0 * gAB
+    assert abs(2.0 * np.mean(b.real * c) / eps - (1.0 + lm * dt * Cc * S) / (1.0 + 2.0 * lm * dt * Cc / chiN)) < 2e-6
+    grid3, cell3, fA3 = (4, 2, 8), (3.0, 4.0, 5.0), 0.3
+    M = int(np.prod(grid3))
+    wm, wp = chiN * (2 * fA3 - 1) / 2, 0.21
+    o = oracle.Oracle(grid3, cell3, 20, "diblock", fA=fA3, chiN=chiN, Cc=Cc, lambda_plus=lp, lambda_minus=lm)
+    o.set_fields(np.full(grid3, wp, np.complex128), np.full(grid3, wm, np.complex128))
+    o.cl_step(dt, 1, 21, 9)
+    a, b = o.get_fields()
+    dV = np.prod(cell3) / M
+    ep = np.sqrt(2 * lp * dt / dV) * np.array([oracle.normal(21, 9, 0, i) for i in range(M)]).reshape(grid3)
+    em = np.sqrt(2 * lm * dt / dV) * np.array([oracle.normal(21, 9, 1, i) for i in range(M)]).reshape(grid3)
+    want_p = 1j * np.fft.ifftn(np.fft.fftn(ep) / (1.0 + lp * dt * Cc * _gD_safe(_k2_grid(grid3, cell3))))
+    assert np.max(np.abs((a - wp) - want_p)) < 1e-12
+    assert np.max(np.abs((b - wm) - em / (1.0 + 2.0 * lm * dt * Cc / chiN))) < 1e-12
+
+
+def test_edwards_H_at_the_homogeneous_saddle(oracle):
+    """Eq. 2 as printed (reading A-13) at Omega* = -iC/B: (B/2) V Omega*^2 = -C^2 V/(2B), ln Q = -C/B,
+    so H = -C^2 V/(2B) + C^2 V/B = C^2 V/(2B); mu = ln C + C/B."""
+    grid, cell, B, Cc = (4, 8, 2), (3.0, 4.0, 5.0), 2.5, 3.0
+    V = float(np.prod(cell))
+    o = oracle.Oracle(grid, cell, 8, "edwards", B=B, Cc=Cc)
+    o.set_fields(np.full(grid, -1j * Cc / B, np.complex128))
+    o.propagate()
+    H, mu, _ = o.operators()
+    assert abs(H - Cc ** 2 * V / (2 * B)) < 1e-12 * V
+    assert abs(mu - (np.log(Cc) + Cc / B)) < 1e-13
+
+
 def test_pressure_kernel_matches_volume_derivative_of_lnQ(oracle):
     """-(2/3V) K = d ln Q / dV at fixed lattice fields (reading A-14; the only pin Pi has: 'parity unpinned')."""
     cfg = inputs.config1(grid=(8, 8, 8), Ns=64)
