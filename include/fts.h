@@ -102,6 +102,20 @@ fts_status fts_cl_step(fts_ctx* ctx, double dt, int scheme, uint64_t seed, uint6
  * DESIGN.md, not printed in the paper: secondary output).  Any pointer may be NULL.  Synchronises `stream`. */
 fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], void* stream);
 
+/* Tuning options (integers), effective from the next fts_propagate / step call; the library reads NO environment
+ * variables.  Unknown keys return FTS_EINVAL.  Keys:
+ *   "march"       how the contour march is issued (fts_march_mode): 0 automatic (default), 1 one launch per phase and
+ *                 step, 2 persistent ticket kernel with per-thread staging (fts_march.cuh), 3 persistent TMA kernel
+ *                 (fts_march2.cuh; cubic grids of 128 or 256 points per side, FTS_EUNSUPPORTED otherwise)
+ *   "slab_bytes"  mode 2: bytes of one L2 slab of the Y1/Z/Y2 phases (0 = one slab)
+ *   "lag"         modes 2-3: slabs / planes between a phase and the phase that consumes it (-1 = default)
+ *   "skew"        mode 3: planes by which q trails q+ inside a step (-1 = default)
+ *   "interleave"  mode 2: alternate the two propagators' phases (default 1)
+ *   "tz"          modes 1-2: pencils per strided tile, 8 or 16 (0 = default)
+ * All modes give bit-identical results. */
+typedef enum { FTS_MARCH_AUTO = 0, FTS_MARCH_LAUNCH = 1, FTS_MARCH_TICKET = 2, FTS_MARCH_TMA = 3 } fts_march_mode;
+fts_status fts_set_option(fts_ctx* ctx, const char* key, long long value);
+
 /* Raw Philox4x32-10 block and the standard normal fts_cl_step draws for (seed, step, field, site), evaluated
  * ON THE DEVICE for n consecutive sites starting at site0; out_dev receives n doubles.  For tests. */
 fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream);

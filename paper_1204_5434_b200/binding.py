@@ -16,7 +16,7 @@ STATUS = {0: "FTS_OK", 1: "FTS_EINVAL", 2: "FTS_ESTATE", 3: "FTS_EWORKSPACE", 4:
 MODELS = {"external": 0, "edwards": 1, "diblock": 2}
 EXPORTS = ["fts_workspace_bytes", "fts_create", "fts_destroy", "fts_set_fields", "fts_get_fields", "fts_propagate",
            "fts_propagate_steps", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
-           "fts_operators", "fts_debug_normals", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
+           "fts_operators", "fts_set_option", "fts_debug_normals", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
 
 
 class FtsParams(C.Structure):
@@ -54,6 +54,7 @@ def lib():
         L.fts_scft_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, dp, dp, vp]
         L.fts_cl_step.argtypes = [vp, C.c_double, C.c_int, C.c_uint64, C.c_uint64, vp]
         L.fts_operators.argtypes = [vp, dp, dp, dp, vp]
+        L.fts_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
         L.fts_debug_normals.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
         L.fts_debug_fma_peak.argtypes = [C.c_int, C.c_int, vp, C.c_size_t, dp, vp]
         L.fts_launch_count.restype = C.c_uint64
@@ -88,7 +89,7 @@ def workspace_bytes(grid, Ns, params, precision="f64"):
 class Fts:
     """One simulation context on the current CUDA device.  Methods mirror the C calls one to one."""
 
-    def __init__(self, grid, cell, Ns, model, precision="f64", device="cuda:0", **kw):
+    def __init__(self, grid, cell, Ns, model, precision="f64", device="cuda:0", options=None, **kw):
         self.grid = tuple(int(v) for v in grid)
         self.Ns = int(Ns)
         self.model = MODELS.get(model, model)
@@ -101,11 +102,18 @@ class Fts:
         h = C.c_void_p()
         g = (C.c_int * 3)(*self.grid)
         c = (C.c_double * 3)(*[float(v) for v in cell])
-        rc = lib().fts_create(g, c, self.Ns, C.byref(self.params), 0 if precision == "f64" else 1,
-                              _p(self.workspace), nbytes, C.byref(h))
+        with torch.cuda.device(self.device):
+            rc = lib().fts_create(g, c, self.Ns, C.byref(self.params), 0 if precision == "f64" else 1,
+                                  _p(self.workspace), nbytes, C.byref(h))
         if rc:
             raise FtsError("fts_create", rc)
         self.h = h
+        for k, v in (options or {}).items():
+            self.set_option(k, v)
+
+    def set_option(self, key, value):
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_set_option(self.h, str(key).encode(), int(value)), f"fts_set_option({key})")
 
     def close(self):
         if getattr(self, "h", None) and _lib is not None:

@@ -13,6 +13,7 @@
 #include "../../include/fts.h"
 #include "fts_kernels.cuh"
 #include "fts_march.cuh"
+#include "fts_march2.cuh"
 
 namespace fts {
 
@@ -34,6 +35,11 @@ struct Ctx {
     unsigned* counters;       // device: completion counters, then ticket and error flag
     size_t counters_bytes;
     int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
+    // options (fts_set_option; no environment variables are read)
+    struct { int march; long long slab_bytes; int lag, interleave, tz, skew; } opt;
+    // TMA march for large cubic grids (fts_march2.cuh)
+    int v2, v2_lag, v2_skew, v2_occ;
+    March2Maps maps;
     std::string err;
 };
 
@@ -41,6 +47,7 @@ static uint64_t g_launches = 0;      // kernels launched by this library since i
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 enum { MARCH_MAXCHUNKS = 64 };
+static int counters_per_step(const int g[3]) { const int a = 2 + 2 * MARCH_MAXCHUNKS, b = 2 + 2 * g[0]; return a > b ? a : b; }
 
 struct Layout {          // the single place that decides where things live in the workspace
     size_t off_tab[3][2], off_tw[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
@@ -61,7 +68,7 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
     Lo.off_kacc = o; o += align_up((size_t)(Ns + 1) * 2 * sizeof(double));
     Lo.off_partial = o; o += align_up(1024 * sizeof(double2));
     Lo.off_phases = o; o += align_up(5 * MARCH_MAXPH * sizeof(Phase));
-    Lo.counters_bytes = align_up((size_t)2 * (Ns + 1) * (2 + 2 * MARCH_MAXCHUNKS) * sizeof(unsigned)) + 256;
+    Lo.counters_bytes = align_up((size_t)2 * (Ns + 1) * counters_per_step(g) * sizeof(unsigned)) + 256;
     Lo.off_counters = o; o += Lo.counters_bytes;
     for (int i = 0; i < 2; ++i) { Lo.off_f[i] = o; o += field; }
     for (int i = 0; i < 2; ++i) { Lo.off_e4[i] = o; o += field; }
@@ -110,12 +117,9 @@ static fts_status validate(const int grid[3], const double* cell, int Ns, const 
 template <class T, int N, int EPT, int TZ>
 static cudaError_t launch_pass_inst(const PassArgs& A, int njobs, cudaStream_t st) {
     typedef PassCfg<T, N, EPT, TZ> Cfg;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    // set on every launch: the attribute is per device, and a process may drive several GPUs
+    cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
     dim3 grid((A.ntiles + Cfg::GPB - 1) / Cfg::GPB, njobs);
     pass_kernel<T, N, EPT, TZ><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
     g_launches += 1;
@@ -183,19 +187,14 @@ static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, M
     typedef MarchCfg<T, N, EPT, TZ> Cfg;
     if (info) { info->threads = Cfg::LAUNCH; info->gpb_s = Cfg::GPB_S; info->gpb_c = Cfg::GPB_C; info->smem = Cfg::SMEM; }
     if (query && !occ) return cudaSuccess;
-    static bool attr_done = false;
-    static size_t extra = std::getenv("FTS_EXTRA_SMEM") ? (size_t)std::atoll(std::getenv("FTS_EXTRA_SMEM")) : 0;   // experiment: lower occupancy
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(march_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(Cfg::SMEM + extra));
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    cudaError_t e = cudaFuncSetAttribute(march_kernel<T, N, EPT, TZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
     if (occ) {
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<T, N, EPT, TZ>, Cfg::LAUNCH, Cfg::SMEM + extra);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<T, N, EPT, TZ>, Cfg::LAUNCH, Cfg::SMEM);
         if (e != cudaSuccess) return e;
     }
     if (query) return cudaSuccess;
-    march_kernel<T, N, EPT, TZ><<<grid, Cfg::LAUNCH, Cfg::SMEM + extra, st>>>(A);
+    march_kernel<T, N, EPT, TZ><<<grid, Cfg::LAUNCH, Cfg::SMEM, st>>>(A);
     g_launches += 1;
     return cudaGetLastError();
 }
@@ -216,8 +215,8 @@ static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool quer
 // length 256 uses 64-byte rows instead: its 128-byte-row CTA (256 + 32 threads) is register-starved (measured: 681 vs 736 us per step at 256^3).
 template <class T> static int tz_used(const Ctx* c) {
     const int full = tz_of<T>();
-    if (std::getenv("FTS_TZ8")) return 8;
-    if (std::getenv("FTS_TZ16") && c->g[2] >= full) return full;
+    if (c->opt.tz == 8) return 8;
+    if (c->opt.tz == 16 && c->g[2] >= full) return full;
     if (sizeof(T) == 4 && (c->g[0] >= 256 || c->g[1] >= 256 || c->g[2] >= 256)) return 8;
     return c->g[2] >= full ? full : 8;
 }
@@ -293,26 +292,23 @@ static fts_status plan_march(Ctx* c) {
     for (int d = 0; d < 3; ++d) CK(launch_march<T>(c, c->g[d], A, 0, true, &mi[d], nullptr, 0));
     int dev = 0; CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
-    const char* mode = std::getenv("FTS_MARCH");
-    c->persistent = (Nx == Ny && Ny == Nz) && !(mode && std::strcmp(mode, "launch") == 0);
+    c->persistent = (Nx == Ny && Ny == Nz) && c->opt.march != FTS_MARCH_LAUNCH;
     // slab size (optional): F and H of the slabs in flight must sit in L2 next to the streaming traffic
     const size_t plane = (size_t)Ny * Nz * c->esz;
     size_t target = ~(size_t)0;        // default: one slab.  Slabs cut HBM traffic from 17 to 13 E*M, but the march is not HBM-bound and
-                                       // coarser phases measure 1.5-3 % faster; FTS_SLAB_BYTES re-enables them
-    if (const char* e = std::getenv("FTS_SLAB_BYTES")) target = (size_t)std::atoll(e);
+                                       // coarser phases measure 1.5-3 % faster; fts_set_option("slab_bytes") re-enables them
+    if (c->opt.slab_bytes > 0) target = (size_t)c->opt.slab_bytes;
     int planes = Nx;
     while (planes > 1 && (size_t)planes * plane > target) planes >>= 1;
     while (Nx / planes > MARCH_MAXCHUNKS) planes <<= 1;
-    if (c->nprop == 1 && planes == Nx && !std::getenv("FTS_SLAB_BYTES")) planes = Nx / 2;      // one propagator: two slabs pipeline Y1/Z/Y2 against each other (-10 % at 64^3)
+    if (c->nprop == 1 && planes == Nx && c->opt.slab_bytes <= 0) planes = Nx / 2;      // one propagator: two slabs pipeline Y1/Z/Y2 against each other (-10 % at 64^3)
     if (!c->persistent) planes = Nx;
     c->planes = planes; c->nchunks = Nx / planes;
-    c->lag = 1;
-    if (const char* e = std::getenv("FTS_LAG")) c->lag = std::atoi(e) >= 0 ? std::atoi(e) : 1;
+    c->lag = c->opt.lag >= 0 ? c->opt.lag : 1;
     std::vector<Phase> all(5 * MARCH_MAXPH, mkphase(0, 0, 0, 0, 0));
     if (c->persistent) {
         phase_counts(c, mi[0], mi[1], mi[2], tz, planes, c->cnt);
-        bool inter = true;
-        if (const char* e = std::getenv("FTS_INTERLEAVE")) inter = std::atoi(e) != 0;
+        const bool inter = c->opt.interleave != 0;
         std::vector<Phase> t = make_template(c->nprop, c->nchunks, c->lag, inter, c->cnt, &c->tickets_per_round);
         if ((int)t.size() > MARCH_MAXPH) { c->err = "march template too long"; return FTS_EINVAL; }
         c->nph = (int)t.size();
@@ -327,10 +323,107 @@ static fts_status plan_march(Ctx* c) {
     return FTS_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// TMA march (fts_march2.cuh): cubic grids with pencil length 128 or 256.  Tensor maps are encoded once per
+// context through the driver entry point (no link-time dependency on libcuda).
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr; cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+static bool v2_shape_ok(const Ctx* c) { return c->g[0] == c->g[1] && c->g[1] == c->g[2] && (c->g[0] == 128 || c->g[0] == 256); }
+
+// one field (or a store of `nslices` fields) seen as [slice][ix][iy][2 Nz scalars]; box = a strided tile along x or along y
+static bool make_tile_map(const Ctx* c, CUtensorMap* m, void* base, int nslices, bool along_x) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint64_t N = (cuuint64_t)c->g[0], es = c->esz;
+    const cuuint64_t dims[4] = {2 * N, N, N, (cuuint64_t)nslices};
+    const cuuint64_t strides[3] = {N * es, N * N * es, N * N * N * es};
+    const cuuint32_t box[4] = {16, along_x ? 1u : (cuuint32_t)N, along_x ? (cuuint32_t)N : 1u, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const bool f64 = c->prec == FTS_F64;
+    return enc(m, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               f64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, f64 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <class T, int N>
+static cudaError_t launch_march2_inst(const Ctx* c, const March2Args& A, int grid, int* occ, cudaStream_t st) {
+    typedef M2Cfg<T, N> Cfg;
+    cudaError_t e = cudaFuncSetAttribute(march2_kernel<T, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    if (occ) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march2_kernel<T, N>, M2_LAUNCH, Cfg::SMEM);
+    march2_kernel<T, N><<<grid, M2_LAUNCH, Cfg::SMEM, st>>>(c->maps, A);
+    g_launches += 1;
+    return cudaGetLastError();
+}
+template <class T>
+static cudaError_t launch_march2(const Ctx* c, const March2Args& A, int grid, int* occ, cudaStream_t st) {
+    return c->g[0] == 256 ? launch_march2_inst<T, 256>(c, A, grid, occ, st) : launch_march2_inst<T, 128>(c, A, grid, occ, st);
+}
+template <class T>
+static long long march2_total(const Ctx* c, int nsteps) {
+    return c->g[0] == 256 ? M2Sched<T, 256>(c->nprop, c->v2_lag, c->v2_skew, nsteps).total() : M2Sched<T, 128>(c->nprop, c->v2_lag, c->v2_skew, nsteps).total();
+}
+
+template <class T>
+static fts_status plan_march2(Ctx* c) {
+    c->v2 = 0;
+    if (!v2_shape_ok(c) || c->opt.march == FTS_MARCH_LAUNCH || c->opt.march == FTS_MARCH_TICKET) return FTS_OK;
+    bool ok = true;
+    for (int b = 0; b < 2 && ok; ++b) {
+        const int pb = b < c->nprop ? b : 0;
+        ok = ok && make_tile_map(c, &c->maps.x[M2_MAP_F + b], c->F[pb], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_H + b], c->H[pb], 1, true) &&
+             make_tile_map(c, &c->maps.x[M2_MAP_E + b], c->e4[b], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_Q + b], c->q[pb], c->Ns + 1, true) &&
+             make_tile_map(c, &c->maps.y[0 + b], c->F[pb], 1, false) && make_tile_map(c, &c->maps.y[2 + b], c->H[pb], 1, false);
+    }
+    if (!ok) {
+        if (c->opt.march == FTS_MARCH_TMA) { c->err = "cuTensorMapEncodeTiled failed or is unavailable"; return FTS_ECUDA; }
+        return FTS_OK;                                    // automatic mode: fall back to the ticket march of fts_march.cuh
+    }
+    const int N = c->g[0], G = N == 256 ? 1 : 2, ppi = N == 256 ? 8 : 16;
+    const int per_slot = c->nprop * (2 * (N / 8 / G) + 2 * (N / ppi) + N / 8 / G);
+    int lag = (2 * c->sms + per_slot - 1) / per_slot + 1;      // a phase and the phase it waits for: more items apart than CTAs in flight
+    if (c->opt.lag >= 0) lag = c->opt.lag;
+    c->v2_lag = lag;
+    c->v2_skew = c->nprop == 2 ? (c->opt.skew >= 0 ? c->opt.skew : lag) : 0;
+    March2Args A; std::memset(&A, 0, sizeof A);
+    CK(launch_march2<T>(c, A, 0, &c->v2_occ, 0));
+    if (c->v2_occ < 1) { c->err = "TMA march kernel does not fit on an SM"; return FTS_ECUDA; }
+    c->v2 = 1;
+    return FTS_OK;
+}
+
+template <class T>
+static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
+    March2Args A; std::memset(&A, 0, sizeof A);
+    for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; A.e4[b] = c->e4[b]; }
+    for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; }
+    A.tw = c->dim[0].tw;
+    A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nprop = c->nprop; A.nsteps = nsteps; A.lag = c->v2_lag; A.skew = c->v2_skew;
+    A.qslot[0] = A.qslot[1] = 0;
+    A.cnt = c->counters; A.ticket = (unsigned*)((char*)c->counters + c->counters_bytes - 256);
+    A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
+    long long grid = (long long)c->v2_occ * c->sms;
+    const long long total = march2_total<T>(c, nsteps);
+    if (grid > total) grid = total;
+    CK(launch_march2<T>(c, A, (int)grid, nullptr, st));
+    return FTS_OK;
+}
+
 template <class T>
 static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     MarchArgs A; fill_march_args<T>(c, A, nsteps);
-    CK(cudaMemsetAsync(c->counters, 0, c->counters_bytes - 128, st));          // counters and ticket; the error flag is sticky
+    CK(cudaMemsetAsync(c->counters, 0, c->counters_bytes - 128, st));          // counters and ticket; the error flag stays until fts_set_fields
+    if (c->v2) return march2_t<T>(c, nsteps, st);
     if (c->persistent) {
         A.nchunks = c->nchunks; A.planes = c->planes;
         A.phases = c->phases; A.nphases = c->nph; A.tickets_per_round = c->tickets_per_round; A.round0 = 0; A.round1 = nsteps;
@@ -574,6 +667,12 @@ static fts_status build_tables(Ctx* c) {
     return FTS_OK;
 }
 
+static fts_status replan(Ctx* c) {
+    fts_status rc = c->prec == FTS_F64 ? plan_march<double>(c) : plan_march<float>(c);
+    if (!rc) rc = c->prec == FTS_F64 ? plan_march2<double>(c) : plan_march2<float>(c);
+    return rc;
+}
+
 }  // namespace fts
 
 using namespace fts;
@@ -622,14 +721,36 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
     }
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->have_fields = c->have_prop = false; c->marched = 0; c->occ = 0;
+    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1;
+    c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
-    if (!rc) rc = DISPATCH(plan_march<double>(c), plan_march<float>(c));
+    if (!rc) rc = replan(c);
     if (rc) { delete c; return rc; }
+    if (cudaDeviceSynchronize() != cudaSuccess) { delete c; return FTS_ECUDA; }      // tables and templates were written on the legacy stream
     *out = c;
     return FTS_OK;
 }
 
 fts_status fts_destroy(fts_ctx* c) { delete c; return FTS_OK; }
+
+fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
+    if (!c || !key) return FTS_EINVAL;
+    const auto old = c->opt;
+    if (!std::strcmp(key, "march")) { if (value < 0 || value > 3) return FTS_EINVAL; c->opt.march = (int)value; }
+    else if (!std::strcmp(key, "slab_bytes")) { if (value < 0) return FTS_EINVAL; c->opt.slab_bytes = value; }
+    else if (!std::strcmp(key, "lag")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.lag = (int)value; }
+    else if (!std::strcmp(key, "skew")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.skew = (int)value; }
+    else if (!std::strcmp(key, "interleave")) c->opt.interleave = value != 0;
+    else if (!std::strcmp(key, "tz")) { if (value != 0 && value != 8 && value != 16) return FTS_EINVAL; c->opt.tz = (int)value; }
+    else return FTS_EINVAL;
+    if (c->opt.march == FTS_MARCH_TMA && !v2_shape_ok(c)) { c->opt = old; return FTS_EUNSUPPORTED; }
+    c->occ = 0;
+    fts_status rc = replan(c);
+    if (rc) return rc;
+    CK(cudaDeviceSynchronize());
+    c->have_prop = false;
+    return FTS_OK;
+}
 
 fts_status fts_set_fields(fts_ctx* c, const void* f0, const void* f1, void* stream) {
     if (!c || !f0 || (c->P.model == FTS_MODEL_DIBLOCK && !f1)) return FTS_EINVAL;

@@ -205,21 +205,20 @@ def test_determinism(B):
 # ------------------------------------------------------------------------------------------------
 # the march schedules (persistent ticket kernel with L2 slabs, stream-ordered launches) and full-size runs
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("env", [{}, {"FTS_MARCH": "launch"}, {"FTS_SLAB_BYTES": "65536"}, {"FTS_SLAB_BYTES": "32768", "FTS_LAG": "3"},
-                                 {"FTS_INTERLEAVE": "0", "FTS_SLAB_BYTES": "131072"}, {"FTS_TZ8": "1"}])
+@pytest.mark.parametrize("opts", [{}, {"march": 1}, {"slab_bytes": 65536}, {"slab_bytes": 32768, "lag": 3},
+                                  {"interleave": 0, "slab_bytes": 131072}, {"tz": 8}])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
-def test_march_schedules_agree(B, oracle, env, precision, monkeypatch):
-    """Cubic 32^3 grid (the persistent kernel's domain): one slab, 8 and 16 slabs with different pipeline lags, and the
-    one-launch-per-phase mode all reproduce the oracle; in fp64 they are also bit-identical to each other."""
-    for k in ("FTS_MARCH", "FTS_SLAB_BYTES", "FTS_LAG", "FTS_TZ8", "FTS_INTERLEAVE", "FTS_EXTRA_SMEM"):
-        monkeypatch.delenv(k, raising=False)
+def test_march_schedules_agree(B, oracle, opts, precision):
+    """Cubic 32^3 grid (the persistent ticket kernel's domain): one slab, 8 and 16 slabs with different pipeline lags, and the
+    one-launch-per-phase mode all reproduce the oracle; they are also bit-identical to each other (fts_set_option)."""
     cfg = inputs.small_diblock(grid=(32, 32, 32), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
     ref, _ = _pair(B, oracle, cfg, precision=precision)
     ref.propagate()
     Qr, par, pbr = ref.density_operators()
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)                      # read by fts_create
     g, o = _pair(B, oracle, cfg, precision=precision)
+    for k, v in opts.items():
+        g.set_option(k, v)
+    g.set_fields(*[torch.from_numpy(np.ascontiguousarray(f)).to("cuda:0").to(g.cdtype) for f in (cfg.f0, cfg.f1)])
     g.propagate(); o.propagate()
     Qg, pa, pb = g.density_operators()
     Qo, oa, ob = o.density_operators()
@@ -227,6 +226,43 @@ def test_march_schedules_agree(B, oracle, env, precision, monkeypatch):
     assert abs(Qg - Qo) <= tol[0] * abs(Qo)
     assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tol[1] and np.max(np.abs(pb.cpu().numpy() - ob)) <= tol[1]
     assert Qg == Qr and torch.equal(pa, par) and torch.equal(pb, pbr)      # the schedule does not change the arithmetic
+
+
+def test_set_option_rejects_bad_values(B):
+    g = B.Fts((16, 16, 16), (4.0,) * 3, 8, "external")
+    for key, val in (("nonsense", 1), ("march", 7), ("tz", 5), ("lag", 1000)):
+        with pytest.raises(B.FtsError) as e:
+            g.set_option(key, val)
+        assert e.value.status == 1                     # FTS_EINVAL
+    with pytest.raises(B.FtsError) as e:
+        g.set_option("march", 3)                       # the TMA march needs a cubic 128^3 or 256^3 grid
+    assert e.value.status == 6                         # FTS_EUNSUPPORTED
+
+
+@pytest.mark.parametrize("precision", ["f64"])
+@pytest.mark.parametrize("model,nsteps", [("diblock", 6), ("diblock", 1), ("external", 4)])
+def test_tma_march_equals_ticket_march_128(B, precision, model, nsteps):
+    """128^3: the TMA march (fts_march2.cuh, automatic choice) and the ticket march (fts_march.cuh) run the same
+    arithmetic in the same order: every slice, F and H are bit-identical.  (Oracle parity of this size: test_full_size_*.)"""
+    Ns = 8
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=(128, 128, 128), cell=(9.0, 10.0, 11.0), Ns=Ns, fA=0.5)
+        kw = dict(fA=cfg.fA, chiN=cfg.chiN, Cc=cfg.C)
+        fields = (cfg.f0, cfg.f1)
+    else:
+        rng = np.random.default_rng(11)
+        fields = ((0.4 + 0.3 * rng.normal(size=(128,) * 3) + 0.2j * rng.normal(size=(128,) * 3)).astype(np.complex128),)
+        kw = {}
+    outs = []
+    for mode in (2, 3):
+        g = B.Fts((128,) * 3, (9.0, 10.0, 11.0), Ns, model, precision=precision, options={"march": mode}, **kw)
+        g.set_fields(*[torch.from_numpy(np.ascontiguousarray(f)).to("cuda:0").to(g.cdtype) for f in fields])
+        g.propagate(nsteps)
+        sl = [g.get_slice(w, j).clone() for w in ((0, 1) if model == "diblock" else (0,)) for j in range(nsteps + 1)]
+        outs.append(sl)
+        del g
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
 
 
 def test_zero_and_one_step_march(B, oracle):
