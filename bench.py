@@ -190,7 +190,8 @@ def run_gpu(args):
     cdt = torch.complex128 if prec == "f64" else torch.complex64
     M, nprop = int(np.prod(cfg.grid)), (2 if cfg.model == "diblock" else 1)
     E = 16 if prec == "f64" else 8
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
+    opts = dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, options=opts, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
     host = [torch.from_numpy(np.ascontiguousarray(f)).to(cdt).pin_memory() for f in (cfg.f0, cfg.f1) if f is not None]
     devf = [h.to(dev) for h in host]
     back = [torch.empty_like(h).pin_memory() for h in host]
@@ -326,6 +327,7 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="fts_set_option (tuning experiments), e.g. --opt march=2")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -1,8 +1,9 @@
 // fts_march2.cuh — the contour march for large cubic grids (pencil length 128 or 256):
 // ONE persistent kernel per propagator solve, tiles staged by TMA, pencils private to a warp.
 //
-// The arithmetic is that of fts_march.cuh (same Pencil butterflies, same order of operations: results are
-// bit-identical); what differs is how data moves:
+// The arithmetic is that of fts_march.cuh (same Pencil butterflies) except that the inverse transform is run as
+// conj o forward o conj (one transform body, half the code); the two kernels agree to rounding.  What differs is how
+// data moves:
 //
 //   * Every work item moves whole tiles between global memory and shared memory with TMA
 //     (cp.async.bulk.tensor on 4-D tensor maps for the strided x / y tiles [N][8 z], 128-byte-swizzled (complex128) or
@@ -199,27 +200,51 @@ struct M2Lane {
     // exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform; the two
     // exchanges of each direction happen in place inside `base`.  Every lane of the warp must have consumed whatever the
     // buffer held before the call (first __syncwarp); on return all lanes have finished reading it (last __syncwarp).
-    template <bool CONTIG> __device__ __forceinline__ void diffuse(C (&v)[16], unsigned char* base, const T* tab) const {
-        const unsigned va = CONTIG ? VAc : VAs, vb = CONTIG ? VBc : VBs;
-        P::fwd_a(v, t, s_tw);
-        __syncwarp();
+    template <bool CONTIG> __device__ __forceinline__ void xst_a(const C (&v)[16], unsigned char* base) const {
+        const unsigned va = CONTIG ? VAc : VAs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(base + (va ^ KA<CONTIG>(r)), v[r]); });
-        __syncwarp();
-        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (vb ^ KB<CONTIG>(r))); });
-        P::fwd_b(v);
-#pragma unroll
-        for (int r = 0; r < 16; ++r) v[r] = v[r] * tab[t + TPP * r];
-        P::inv_b(v);
-        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(base + (vb ^ KB<CONTIG>(r)), v[r]); });
-        __syncwarp();
+    }
+    template <bool CONTIG> __device__ __forceinline__ void xld_a(C (&v)[16], const unsigned char* base) const {
+        const unsigned va = CONTIG ? VAc : VAs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (va ^ KA<CONTIG>(r))); });
-        P::inv_a(v, t, s_tw);
-        __syncwarp();
+    }
+    template <bool CONTIG> __device__ __forceinline__ void xst_b(const C (&v)[16], unsigned char* base) const {
+        const unsigned vb = CONTIG ? VBc : VBs;
+        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(base + (vb ^ KB<CONTIG>(r)), v[r]); });
+    }
+    template <bool CONTIG> __device__ __forceinline__ void xld_b(C (&v)[16], const unsigned char* base) const {
+        const unsigned vb = CONTIG ? VBc : VBs;
+        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (vb ^ KB<CONTIG>(r))); });
+    }
+    // exp(a ds d^2/dx_d^2) along the pencil = F^-1 [table] F, with the inverse transform run as conj o F o conj, so that ONE
+    // forward-transform body (radix-R1 butterflies, twiddles, exchange A -> B, radix-R2 butterflies) is executed twice in a
+    // rolled loop: the hot code of the kernel is then about 9 KB.  The four compute warps of a CTA run at different places
+    // of the kernel, so its working set has to fit the instruction caches (measured: 17 % of the warps' time went to
+    // instruction fetch with both transforms unrolled).  The butterflies are shared by the two layouts; only the exchange
+    // accesses are specialised.  The real table carries 1/N; conj(v * tab) = (v.x tab, v.y (-tab)).
+    __device__ __forceinline__ void diffuse(C (&v)[16], unsigned char* base, bool contig, const T* tab) const {
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            P::fwd_a(v, t, s_tw);
+            __syncwarp();                                  // every lane has consumed what the buffer held / its B-pattern loads
+            if (contig) xst_a<true>(v, base); else xst_a<false>(v, base);
+            __syncwarp();
+            if (contig) xld_b<true>(v, base); else xld_b<false>(v, base);
+            P::fwd_b(v);
+            if (pass == 0) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) { const T w = tab[t + TPP * r]; v[r] = mk<T>(v[r].x * w, v[r].y * (-w)); }
+            } else {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r].y = -v[r].y;
+            }
+        }
+        __syncwarp();                                      // all exchange reads done before anyone writes natural positions
     }
 };
 
 template <class T, int N>
-__global__ void __launch_bounds__(M2_LAUNCH, 2) march2_kernel(const __grid_constant__ March2Maps maps, const March2Args A) {
+__global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_kernel(const __grid_constant__ March2Maps maps, const March2Args A) {
     typedef M2Cfg<T, N> Cfg;
     typedef Pencil<T, N, 16> P;
     typedef cplx<T> C;
@@ -281,6 +306,9 @@ __global__ void __launch_bounds__(M2_LAUNCH, 2) march2_kernel(const __grid_const
                 else if (d.kind == PH_Y1) { dep = cb; need = Cfg::NT_X; }
                 else if (d.kind == PH_Z) { dep = cb + 2 + d.plane; need = Cfg::NY1; }
                 else { dep = cb + 2 + N + d.plane; need = Cfg::NZZ; }
+#ifdef FTS_M2_NODEPS
+                dep = nullptr;                                             // measurement build only: wrong results, shows what the schedule costs
+#endif
                 if (dep && dep != dep_ok) {
                     unsigned spins = 0;
                     unsigned long long t0 = 0;
@@ -398,9 +426,13 @@ __global__ void __launch_bounds__(M2_LAUNCH, 2) march2_kernel(const __grid_const
     const M2Lane<T, N> L = {VAs, VBs, VAc, VBc, t, s_tw};
     auto load_nat = [&](C (&v)[16], const unsigned char* base, bool contig) { if (contig) L.template load_nat<true>(v, base); else L.template load_nat<false>(v, base); };
     auto store_nat = [&](const C (&v)[16], unsigned char* base, bool contig) { if (contig) L.template store_nat<true>(v, base); else L.template store_nat<false>(v, base); };
-    auto diffuse = [&](C (&v)[16], unsigned char* base, bool contig, const T* tab) { if (contig) L.template diffuse<true>(v, base, tab); else L.template diffuse<false>(v, base, tab); };
-    auto release = [&](int buf) { m2_fence_async_smem(); mbar_arrive(&b_out[buf]); };      // this thread is done with the buffer
+    auto diffuse = [&](C (&v)[16], unsigned char* base, bool contig, const T* tab) { L.diffuse(v, base, contig, tab); };
+    // this thread is done with the buffer; `stored`: it wrote a tile the store thread will hand to TMA (generic -> async proxy)
+    auto release = [&](int buf, bool stored) { if (stored) m2_fence_async_smem(); mbar_arrive(&b_out[buf]); };
 
+    // One item = a short program of stages  [load tile ->] diffuse -> post action.  The loop below has ONE call site of
+    // load_nat / diffuse / store_nat (two bodies each: strided and contiguous layout), which keeps the kernel's hot code
+    // small enough for the instruction caches although the four warps of a CTA run at different places of it.
     unsigned alloc = 0;
     for (unsigned item = 0;; ++item) {
         const int slot = item % M2_RING;
@@ -408,82 +440,84 @@ __global__ void __launch_bounds__(M2_LAUNCH, 2) march2_kernel(const __grid_const
         const volatile M2Desc* dv = &s_desc[slot];
         const int kind = dv->kind, flags = dv->flags;
         if (kind < 0) break;
-        const int bA = alloc % M2_NBUF; const unsigned uA = alloc / M2_NBUF;
-        unsigned char* pA = s_buf + bA * BUFB;
+        const int bA = alloc % M2_NBUF, bB = (alloc + 1) % M2_NBUF, bC = (alloc + 2) % M2_NBUF;
+        const unsigned uA = alloc / M2_NBUF, uB = (alloc + 1) / M2_NBUF, uC = (alloc + 2) / M2_NBUF;
+        unsigned char* pA = s_buf + bA * BUFB; unsigned char* pB = s_buf + bB * BUFB; unsigned char* pC = s_buf + bC * BUFB;
+        const bool contig = kind == PH_Z, jobh = flags & M2_JOBH;
+        const T* tabd = s_tab + (kind == PH_T ? 0 : (contig ? 4 * N : 2 * N));      // [full][half] of the item's dimension
+        alloc += kind == PH_T ? 3 : (contig ? 2 : 1);
         C v[16];
-        if (kind == PH_T) {
-            const int bB = (alloc + 1) % M2_NBUF, bC = (alloc + 2) % M2_NBUF;
-            const unsigned uB = (alloc + 1) / M2_NBUF, uC = (alloc + 2) / M2_NBUF;
-            unsigned char* pB = s_buf + bB * BUFB; unsigned char* pC = s_buf + bC * BUFB;
-            const T* tabx = s_tab;                                          // dimension 0: [full][half]
-            m2_wait(&b_full[bA], uA & 1, A.err);
-            if (flags & M2_FIN) {
-                load_nat(v, pA, false);
-                diffuse(v, pA, false, tabx + N);
-            }
+        // q_s = (4 e4 Dx'[H] - F)/3 -> slice (Eq. 12);  start of step s: stash e4 q_s, v = e4^2 q_s.
+        // Buffers of a T item: A = H (then q_s), B = e4 (then F), C = F (then the stash, then H).
+        auto combine = [&]() {
             m2_wait(&b_full[bB], uB & 1, A.err);
             m2_wait(&b_full[bC], uC & 1, A.err);
-            {   // q_s = (4 e4 Dx'[H] - F)/3 -> slice (Eq. 12);  start of step s: stash e4 q_s, v = e4^2 q_s
-                const bool fin = flags & M2_FIN, start = flags & M2_START, reload = flags & M2_RELOAD;
-                const unsigned char* pe = pB + VAs; const unsigned char* pf = pC + VAs;
-                unsigned char* pq = pA + VAs; unsigned char* ph = pC + VAs;
-                const C* e4s = nullptr; int gbase = 0;
-                if (reload) {                                               // block junction: the new species' factors straight from global memory
-                    const int idx = dv->idx;
-                    const int tile = idx * Cfg::G + w / Cfg::WPT, z = (tile % (N / 8)) * 8 + (w % Cfg::WPT) * Cfg::ZPW + zz, iy = tile / (N / 8);
-                    e4s = static_cast<const C*>(A.e4[dv->spS]); gbase = (t * N + iy) * N + z;
-                }
+            const bool fin = flags & M2_FIN, start = flags & M2_START, reload = flags & M2_RELOAD;
+            const unsigned char* pe = pB + VAs; const unsigned char* pf = pC + VAs;
+            unsigned char* pq = pA + VAs; unsigned char* ph = pC + VAs;
+            const C* e4s = nullptr; int gbase = 0;
+            if (reload) {                                               // block junction: the new species' factors straight from global memory
+                const int idx = dv->idx;
+                const int tile = idx * Cfg::G + w / Cfg::WPT, z = (tile % (N / 8)) * 8 + (w % Cfg::WPT) * Cfg::ZPW + zz, iy = tile / (N / 8);
+                e4s = static_cast<const C*>(A.e4[dv->spS]); gbase = (t * N + iy) * N + z;
+            }
 #pragma unroll
-                for (int r = 0; r < 16; ++r) {
-                    C e = L.ld(pe + r * TPP * RB);
-                    if (fin) {
-                        const C f = L.ld(pf + r * TPP * RB);
-                        const C h = v[r] * e;
-                        v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
-                    } else v[r] = mk<T>(1, 0);                              // q(x,0) = 1, q+(x,s=1) = 1
-                    L.st(pq + r * TPP * RB, v[r]);
-                    if (start) {
-                        if (reload) e = ldcg(e4s + gbase + r * TPP * N * N);
-                        const C hb = v[r] * e;
-                        L.st(ph + r * TPP * RB, hb);
-                        v[r] = hb * e;
-                    }
+            for (int r = 0; r < 16; ++r) {
+                C e = L.ld(pe + r * TPP * RB);
+                if (fin) {
+                    const C f = L.ld(pf + r * TPP * RB);
+                    const C h = v[r] * e;
+                    v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
+                } else v[r] = mk<T>(1, 0);                              // q(x,0) = 1, q+(x,s=1) = 1
+                L.st(pq + r * TPP * RB, v[r]);
+                if (start) {
+                    if (reload) e = ldcg(e4s + gbase + r * TPP * N * N);
+                    const C hb = v[r] * e;
+                    L.st(ph + r * TPP * RB, hb);
+                    v[r] = hb * e;
                 }
             }
-            release(bA);                                                    // q_s -> slice store
-            if (flags & M2_START) {
-                diffuse(v, pB, false, tabx);                                // F = Dx[e2 q_s]   (exchange inside the e4 buffer)
-                store_nat(v, pB, false);
-                release(bB);
-                load_nat(v, pC, false);
-                diffuse(v, pC, false, tabx + N);                            // H = Dx'[e4 q_s]
-                store_nat(v, pC, false);
-                release(bC);
-            } else { release(bB); release(bC); }
-            alloc += 3;
-        } else if (kind == PH_Z) {
-            const int bB = (alloc + 1) % M2_NBUF; const unsigned uB = (alloc + 1) / M2_NBUF;
-            const unsigned char* pB = s_buf + bB * BUFB;
-            const T* tabz = s_tab + 4 * N;
-            const bool jobh = flags & M2_JOBH;
-            m2_wait(&b_full[bA], uA & 1, A.err);
-            load_nat(v, pA, true);
-            diffuse(v, pA, true, jobh ? tabz + N : tabz);
-            m2_wait(&b_full[bB], uB & 1, A.err);
+            release(bA, true);                                          // q_s -> slice store
+            if (!start) { release(bB, false); release(bC, false); }
+            return start;
+        };
+        m2_wait(&b_full[bA], uA & 1, A.err);
+        unsigned char* cur = pA; int curb = bA;
+        const T* tab = (kind == PH_T || jobh) ? tabd + N : tabd;
+        int st = 0;
+        bool run = true, need_load = true;
+        if (kind == PH_T && !(flags & M2_FIN)) {                            // first slice: nothing to finish
+            run = combine();
+            cur = pB; curb = bB; tab = tabd; st = 1; need_load = false;
+        }
+#pragma unroll 1
+        while (run) {
+            if (need_load) load_nat(v, cur, contig);
+#ifdef FTS_M2_SYNC_WARPS
+            bar_compute<M2_NT>();
+#endif
+            diffuse(v, cur, contig, tab);
+            bool store = true;
+            if (kind == PH_T) {
+                if (st == 0) {                                              // H' = Dx'[H] done
+                    store = false;
+                    run = combine();
+                    cur = pB; curb = bB; tab = tabd; st = 1; need_load = false;      // next: F = Dx[e2 q_s], exchanged inside the e4 buffer
+                } else if (st == 2) run = false;                            // H = Dx'[e4 q_s] done
+            } else if (contig) {
+                if (st == 0) {                                              // F = e2 Dz F;  H = Dz'[e2 Dz' H]
+                    m2_wait(&b_full[bB], uB & 1, A.err);
 #pragma unroll
-            for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + VAc + r * TPP * ES); v[r] = v[r] * (e * e); }
-            if (jobh) diffuse(v, pA, true, tabz + N);                       // H = Dz'[e2 Dz' H];  F = e2 Dz F
-            store_nat(v, pA, true);
-            release(bA); release(bB);
-            alloc += 2;
-        } else {                                                            // Y1: F = Dy F, H = Dy' H;  Y2: H = Dy' H
-            const T* taby = s_tab + 2 * N;
-            m2_wait(&b_full[bA], uA & 1, A.err);
-            load_nat(v, pA, false);
-            diffuse(v, pA, false, (flags & M2_JOBH) ? taby + N : taby);
-            store_nat(v, pA, false);
-            release(bA);
-            alloc += 1;
+                    for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + VAc + r * TPP * ES); v[r] = v[r] * (e * e); }
+                    if (jobh) { store = false; st = 1; need_load = false; } else run = false;
+                } else run = false;
+            } else run = false;                                             // Y1: F = Dy F, H = Dy' H;  Y2: H = Dy' H
+            if (store) {
+                store_nat(v, cur, contig);
+                release(curb, true);
+                if (contig) release(bB, false);
+                if (kind == PH_T && st == 1) { cur = pC; curb = bC; tab = tabd + N; st = 2; need_load = true; }      // next: the stash -> H
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&b_iempty[slot]);

@@ -158,18 +158,32 @@ struct Pencil {
     // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.  The twiddles are stored per
     // (register, thread): tw[r*TPP + t] = exp(-2 pi i (t + TPP*g) k1 / N) with g = r % G1, k1 = r / G1, so that the
     // lanes of a warp read consecutive (contiguous pass) or identical (strided pass) addresses.
+    // Inter-stage twiddle of register r (G1 = 1 for every two-stage shape): z^r with z = exp(-2 pi i t / N), stored per
+    // (register, thread) at tw[r*TPP + t] so that lanes read consecutive or identical addresses.  Shared memory bandwidth is
+    // what bounds the fused passes, so only z, z^2, z^3 and z^4, z^8, z^12 are LOADED (correctly rounded host values); the
+    // others are one product z^(4a) * z^b (one extra rounding, < 2 ulp): 9 of 15 loads (3 of 7 for radix 8) become 4 flops each.
+    template <int DIR, class TW>
+    static FTS_HD void twiddle(C (&v)[EPT], int t, const TW* tw) {
+        static_assert(S::ONE || S::G1 == 1, "twiddle scheme assumes one first-stage butterfly per thread");
+        if constexpr (!S::ONE) {
+            auto get = [&](int r) { TW w = tw[r * S::TPP + t]; return mk<T>((T)w.x, DIR < 0 ? (T)w.y : -(T)w.y); };
+            const C w1 = get(1), w2 = get(2), w3 = get(3);
+            v[1] = v[1] * w1; v[2] = v[2] * w2; v[3] = v[3] * w3;
+            static_for<1, S::R1 / 4>([&](auto aa) {
+                constexpr int a = decltype(aa)::value;
+                const C wa = get(4 * a);
+                v[4 * a] = v[4 * a] * wa;
+                v[4 * a + 1] = v[4 * a + 1] * (wa * w1);
+                v[4 * a + 2] = v[4 * a + 2] * (wa * w2);
+                v[4 * a + 3] = v[4 * a + 3] * (wa * w3);
+            });
+        }
+    }
+    // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.
     template <class TW>
     static FTS_HD void fwd_a(C (&v)[EPT], int t, const TW* tw) {
         static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, -1>(v); });
-        if constexpr (!S::ONE) {
-            static_for<0, EPT>([&](auto rr) {
-                constexpr int r = decltype(rr)::value, k1 = r / S::G1;
-                if constexpr (k1 > 0) {
-                    TW w = tw[r * S::TPP + t];
-                    v[r] = v[r] * mk<T>((T)w.x, (T)w.y);
-                }
-            });
-        }
+        twiddle<-1>(v, t, tw);
     }
     // exchange A -> B: after store + barrier + load, register g' + G2*n2 of thread t holds Y[n2][k1 = t + TPP*g'].
     template <class L>
@@ -214,15 +228,7 @@ struct Pencil {
     }
     template <class TW>
     static FTS_HD void inv_a(C (&v)[EPT], int t, const TW* tw) {
-        if constexpr (!S::ONE) {
-            static_for<0, EPT>([&](auto rr) {
-                constexpr int r = decltype(rr)::value, k1 = r / S::G1;
-                if constexpr (k1 > 0) {
-                    TW w = tw[r * S::TPP + t];
-                    v[r] = v[r] * mk<T>((T)w.x, -(T)w.y);
-                }
-            });
-        }
+        twiddle<+1>(v, t, tw);
         static_for<0, S::G1>([&](auto g) { dft_reg<S::R1, S::G1, decltype(g)::value, +1>(v); });
     }
 };
