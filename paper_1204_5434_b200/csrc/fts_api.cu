@@ -391,13 +391,18 @@ static fts_status plan_march2(Ctx* c) {
     }
     const int N = c->g[0], G = N == 256 ? 1 : 2, ppi = N == 256 ? 8 : 16;
     const int per_slot = c->nprop * (2 * (N / 8 / G) + 2 * (N / ppi) + N / 8 / G);
-    int lag = (2 * c->sms + per_slot - 1) / per_slot + 1;      // a phase and the phase it waits for: more items apart than CTAs in flight
-    if (c->opt.lag >= 0) lag = c->opt.lag;
-    c->v2_lag = lag;
-    c->v2_skew = c->nprop == 2 ? (c->opt.skew >= 0 ? c->opt.skew : lag) : 0;
     March2Args A; std::memset(&A, 0, sizeof A);
     CK(launch_march2<T>(c, A, 0, &c->v2_occ, 0));
     if (c->v2_occ < 1) { c->err = "TMA march kernel does not fit on an SM"; return FTS_ECUDA; }
+    // A phase and the phase that consumes it must be further apart in ticket order than the tickets in flight: each CTA
+    // holds up to 5 (one computing, two staged, one waiting for a buffer, one drawn ahead).  Measured on B200: the march
+    // time is flat from 1.25x that distance on (lag 24-32 at 128^3, 4-6 at 256^3) and rises below it.
+    const int inflight = 5 * c->v2_occ * c->sms;
+    int lag = (5 * inflight / 4 + per_slot - 1) / per_slot;
+    if (lag > 48) lag = 48;
+    if (c->opt.lag >= 0) lag = c->opt.lag;
+    c->v2_lag = lag;
+    c->v2_skew = c->nprop == 2 ? (c->opt.skew >= 0 ? c->opt.skew : lag) : 0;
     c->v2 = 1;
     return FTS_OK;
 }

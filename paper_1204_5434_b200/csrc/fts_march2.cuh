@@ -69,14 +69,18 @@ struct M2Cfg {
     static constexpr int G = 4 / WPT;                       // strided tiles per item
     static constexpr int PPI = 4 * ZPW;                     // contiguous pencils per item
     static constexpr int TILEB = N * RB;
-    static constexpr int BUFB = 2048 * ES;                  // one buffer = one item's tile(s) = 128 threads x 16 values
+    // contiguous pencils in shared memory: stride N*ES, plus 64 bytes where a warp's pencils would otherwise fall on the
+    // same banks (complex64, N = 128: four 1 KB pencils per warp, 64 bytes per pencil and access)
+    static constexpr int PPAD = (ES == 8 && N == 128) ? 64 : 0;
+    static constexpr int PSTR = N * ES + PPAD;
+    static constexpr int BUFB = 2048 * ES + PPI * PPAD;     // one buffer = one item's tile(s) = 128 threads x 16 values
     static constexpr int NT_X = (N * N / 8) / G;            // items of a T phase
     static constexpr int NY = (N / 8) / G;                  // y items per plane and job
     static constexpr int NZ = N / PPI;                      // z items per plane and job
     static constexpr int NY1 = 2 * NY, NZZ = 2 * NZ, NY2 = NY;
     static constexpr int C2 = 2 + 2 * N;                    // counters per (propagator, step)
     static constexpr size_t SMEM = (size_t)M2_NBUF * BUFB + (size_t)N * ES + (size_t)6 * N * sizeof(T) + 512;
-    static_assert(S::G1 == 1 && TPP == R2 && G * TILEB == BUFB && PPI * N * ES == BUFB, "unsupported shape");
+    static_assert(S::G1 == 1 && TPP == R2 && G * TILEB == 2048 * ES && PPI * N * ES == 2048 * ES && BUFB % 1024 == 0, "unsupported shape");
 };
 
 __host__ __device__ constexpr unsigned m2_swz(unsigned L, unsigned m) { return L ^ (((L >> 7) & m) << 4); }
@@ -179,7 +183,8 @@ struct M2Lane {
     typedef M2Cfg<T, N> Cfg;
     typedef Pencil<T, N, 16> P;
     typedef cplx<T> C;
-    unsigned VAs, VBs, VAc, VBc;
+    unsigned VAs, VBs, VAc, VBc;         // thread part of the address inside a tile / a pencil
+    unsigned offs, offc;                 // this warp's strided sub-tile / this lane's contiguous pencil inside a buffer
     int t;
     const C* s_tw;
     static constexpr int TPP = Cfg::TPP, R2 = Cfg::R2, G2 = Cfg::G2, ES = Cfg::ES, RB = Cfg::RB;
@@ -190,30 +195,30 @@ struct M2Lane {
     static __device__ __forceinline__ void st(unsigned char* p, C v) { *reinterpret_cast<C*>(p) = v; }
 
     template <bool CONTIG> __device__ __forceinline__ void load_nat(C (&v)[16], const unsigned char* base) const {
-        const unsigned char* p = base + (CONTIG ? VAc : VAs);
+        const unsigned char* p = base + (CONTIG ? offc + VAc : offs + VAs);
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(p + r * TPP * stride<CONTIG>()); });
     }
     template <bool CONTIG> __device__ __forceinline__ void store_nat(const C (&v)[16], unsigned char* base) const {
-        unsigned char* p = base + (CONTIG ? VAc : VAs);
+        unsigned char* p = base + (CONTIG ? offc + VAc : offs + VAs);
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(p + r * TPP * stride<CONTIG>(), v[r]); });
     }
     // exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform; the two
     // exchanges of each direction happen in place inside `base`.  Every lane of the warp must have consumed whatever the
     // buffer held before the call (first __syncwarp); on return all lanes have finished reading it (last __syncwarp).
     template <bool CONTIG> __device__ __forceinline__ void xst_a(const C (&v)[16], unsigned char* base) const {
-        const unsigned va = CONTIG ? VAc : VAs;
+        const unsigned va = CONTIG ? VAc : VAs; base += CONTIG ? offc : offs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(base + (va ^ KA<CONTIG>(r)), v[r]); });
     }
     template <bool CONTIG> __device__ __forceinline__ void xld_a(C (&v)[16], const unsigned char* base) const {
-        const unsigned va = CONTIG ? VAc : VAs;
+        const unsigned va = CONTIG ? VAc : VAs; base += CONTIG ? offc : offs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (va ^ KA<CONTIG>(r))); });
     }
     template <bool CONTIG> __device__ __forceinline__ void xst_b(const C (&v)[16], unsigned char* base) const {
-        const unsigned vb = CONTIG ? VBc : VBs;
+        const unsigned vb = CONTIG ? VBc : VBs; base += CONTIG ? offc : offs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; st(base + (vb ^ KB<CONTIG>(r)), v[r]); });
     }
     template <bool CONTIG> __device__ __forceinline__ void xld_b(C (&v)[16], const unsigned char* base) const {
-        const unsigned vb = CONTIG ? VBc : VBs;
+        const unsigned vb = CONTIG ? VBc : VBs; base += CONTIG ? offc : offs;
         static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (vb ^ KB<CONTIG>(r))); });
     }
     // exp(a ds d^2/dx_d^2) along the pencil = F^-1 [table] F, with the inverse transform run as conj o F o conj, so that ONE
@@ -244,12 +249,13 @@ struct M2Lane {
 };
 
 template <class T, int N>
-__global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_kernel(const __grid_constant__ March2Maps maps, const March2Args A) {
+__global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_kernel(const __grid_constant__ March2Maps maps, const March2Args A) {
     typedef M2Cfg<T, N> Cfg;
     typedef Pencil<T, N, 16> P;
     typedef cplx<T> C;
-    constexpr int TPP = Cfg::TPP, R2 = Cfg::R2, G2 = Cfg::G2, ES = Cfg::ES, RB = Cfg::RB, BUFB = Cfg::BUFB;
+    constexpr int TPP = Cfg::TPP, R2 = Cfg::R2, ES = Cfg::ES, RB = Cfg::RB, BUFB = Cfg::BUFB;
     constexpr unsigned SWM = Cfg::SWM;
+    constexpr unsigned TILE2 = 2048 * ES;                                // bytes one item moves per buffer
 
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* s_buf = smem;
@@ -343,16 +349,17 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_ke
                         const bool load = k == 1 ? true : !(d.flags & M2_FIRST);
                         if (!load) mbar_arrive(&b_full[buf]);
                         else {
-                            m2_expect_tx(&b_full[buf], BUFB);
+                            m2_expect_tx(&b_full[buf], TILE2);
                             const CUtensorMap* mp = &maps.x[k == 0 ? M2_MAP_H + d.b : (k == 1 ? M2_MAP_E + d.spE : M2_MAP_F + d.b)];
                             for (int g = 0; g < Cfg::G; ++g) { int c0, c1; xcoord(d.idx, g, c0, c1); m2_tma_load4(dst + g * Cfg::TILEB, mp, c0, c1, 0, 0, &b_full[buf]); }
                         }
                     } else if (d.kind == PH_Z) {
-                        m2_expect_tx(&b_full[buf], BUFB);
+                        m2_expect_tx(&b_full[buf], TILE2);
                         const char* src = k == 0 ? static_cast<const char*>((d.flags & M2_JOBH) ? A.H[d.b] : A.F[d.b]) : static_cast<const char*>(A.e4[d.spE]);
-                        m2_bulk_load(dst, src + zoffset(d.plane, d.idx), BUFB, &b_full[buf]);
+                        if constexpr (Cfg::PPAD == 0) m2_bulk_load(dst, src + zoffset(d.plane, d.idx), TILE2, &b_full[buf]);
+                        else for (int p = 0; p < Cfg::PPI; ++p) m2_bulk_load(dst + p * Cfg::PSTR, src + zoffset(d.plane, d.idx) + (size_t)p * N * ES, N * ES, &b_full[buf]);
                     } else {
-                        m2_expect_tx(&b_full[buf], BUFB);
+                        m2_expect_tx(&b_full[buf], TILE2);
                         const CUtensorMap* mp = &maps.y[((d.flags & M2_JOBH) ? 2 : 0) + d.b];
                         for (int g = 0; g < Cfg::G; ++g) m2_tma_load4(dst + g * Cfg::TILEB, mp, (d.idx * Cfg::G + g) * 16, 0, d.plane, 0, &b_full[buf]);
                     }
@@ -393,7 +400,11 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_ke
                     }
                 } else if (d.kind == PH_Z) {
                     if (k == 1) store = false;
-                    else m2_bulk_store(static_cast<char*>((d.flags & M2_JOBH) ? A.H[d.b] : A.F[d.b]) + zoffset(d.plane, d.idx), src, BUFB);
+                    else {
+                        char* dst = static_cast<char*>((d.flags & M2_JOBH) ? A.H[d.b] : A.F[d.b]) + zoffset(d.plane, d.idx);
+                        if constexpr (Cfg::PPAD == 0) m2_bulk_store(dst, src, TILE2);
+                        else for (int p = 0; p < Cfg::PPI; ++p) m2_bulk_store(dst + (size_t)p * N * ES, src + p * Cfg::PSTR, N * ES);
+                    }
                 } else {
                     const CUtensorMap* mp = &maps.y[((d.flags & M2_JOBH) ? 2 : 0) + d.b];
                     for (int g = 0; g < Cfg::G; ++g) m2_tma_store4(mp, (d.idx * Cfg::G + g) * 16, 0, d.plane, 0, src + g * Cfg::TILEB);
@@ -419,11 +430,11 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_ke
     // strided tiles: sub-tile g = w / WPT, z = (w % WPT) * ZPW + zz; contiguous: pencil p = w * ZPW + zz
     const unsigned vs_l = (unsigned)(t * RB + ((w % Cfg::WPT) * Cfg::ZPW + zz) * ES);
     const unsigned sub = (unsigned)((w / Cfg::WPT) * Cfg::TILEB);
-    const unsigned VAs = sub + m2_swz(vs_l, SWM), VBs = sub + m2_swz((unsigned)((t * R2 + t) * RB) + (vs_l & (RB - 1)), SWM);
-    const unsigned pen = (unsigned)((w * Cfg::ZPW + zz) * N * ES);
-    const unsigned VAc = pen + t * ES, VBc = pen + (t * R2 + t) * ES;
+    const unsigned VAs = m2_swz(vs_l, SWM), VBs = m2_swz((unsigned)((t * R2 + t) * RB) + (vs_l & (RB - 1)), SWM);
+    const unsigned pen = (unsigned)((w * Cfg::ZPW + zz) * Cfg::PSTR);
+    const unsigned VAc = t * ES, VBc = (t * R2 + t) * ES;
 
-    const M2Lane<T, N> L = {VAs, VBs, VAc, VBc, t, s_tw};
+    const M2Lane<T, N> L = {VAs, VBs, VAc, VBc, sub, pen, t, s_tw};
     auto load_nat = [&](C (&v)[16], const unsigned char* base, bool contig) { if (contig) L.template load_nat<true>(v, base); else L.template load_nat<false>(v, base); };
     auto store_nat = [&](const C (&v)[16], unsigned char* base, bool contig) { if (contig) L.template store_nat<true>(v, base); else L.template store_nat<false>(v, base); };
     auto diffuse = [&](C (&v)[16], unsigned char* base, bool contig, const T* tab) { L.diffuse(v, base, contig, tab); };
@@ -453,8 +464,8 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_ke
             m2_wait(&b_full[bB], uB & 1, A.err);
             m2_wait(&b_full[bC], uC & 1, A.err);
             const bool fin = flags & M2_FIN, start = flags & M2_START, reload = flags & M2_RELOAD;
-            const unsigned char* pe = pB + VAs; const unsigned char* pf = pC + VAs;
-            unsigned char* pq = pA + VAs; unsigned char* ph = pC + VAs;
+            const unsigned char* pe = pB + sub + VAs; const unsigned char* pf = pC + sub + VAs;
+            unsigned char* pq = pA + sub + VAs; unsigned char* ph = pC + sub + VAs;
             const C* e4s = nullptr; int gbase = 0;
             if (reload) {                                               // block junction: the new species' factors straight from global memory
                 const int idx = dv->idx;
@@ -508,7 +519,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 3)) march2_ke
                 if (st == 0) {                                              // F = e2 Dz F;  H = Dz'[e2 Dz' H]
                     m2_wait(&b_full[bB], uB & 1, A.err);
 #pragma unroll
-                    for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + VAc + r * TPP * ES); v[r] = v[r] * (e * e); }
+                    for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + pen + VAc + r * TPP * ES); v[r] = v[r] * (e * e); }
                     if (jobh) { store = false; st = 1; need_load = false; } else run = false;
                 } else run = false;
             } else run = false;                                             // Y1: F = Dy F, H = Dy' H;  Y2: H = Dy' H

@@ -242,8 +242,9 @@ def test_set_option_rejects_bad_values(B):
 @pytest.mark.parametrize("precision", ["f64"])
 @pytest.mark.parametrize("model,nsteps", [("diblock", 6), ("diblock", 1), ("external", 4)])
 def test_tma_march_equals_ticket_march_128(B, precision, model, nsteps):
-    """128^3: the TMA march (fts_march2.cuh, automatic choice) and the ticket march (fts_march.cuh) run the same
-    arithmetic in the same order: every slice, F and H are bit-identical.  (Oracle parity of this size: test_full_size_*.)"""
+    """128^3: the TMA march (fts_march2.cuh, automatic choice) and the ticket march (fts_march.cuh) use the same butterflies;
+    the TMA march runs its inverse transform as conj o forward o conj, so the two agree to rounding on every slice, including
+    across the block junction.  (Oracle parity of this size: test_full_size_*.)"""
     Ns = 8
     if model == "diblock":
         cfg = inputs.small_diblock(grid=(128, 128, 128), cell=(9.0, 10.0, 11.0), Ns=Ns, fA=0.5)
@@ -262,7 +263,7 @@ def test_tma_march_equals_ticket_march_128(B, precision, model, nsteps):
         outs.append(sl)
         del g
     for a, b in zip(*outs):
-        assert torch.equal(a, b)
+        assert (a - b).abs().max().item() < 1e-13
 
 
 def test_zero_and_one_step_march(B, oracle):
