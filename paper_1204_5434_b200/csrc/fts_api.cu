@@ -19,7 +19,7 @@ namespace fts {
 
 static const long double kPiL = 3.14159265358979323846264338327950288L;
 
-struct DimTables { void* tab[2]; void* tw; double* k2; };
+struct DimTables { void* tab[2]; void* tw; void* tw2; double* k2; };
 
 struct Ctx {
     int g[3]; double L[3]; int Ns; fts_params P; fts_precision prec;
@@ -50,7 +50,7 @@ enum { MARCH_MAXCHUNKS = 64 };
 static int counters_per_step(const int g[3]) { const int a = 2 + 2 * MARCH_MAXCHUNKS, b = 2 + 2 * g[0]; return a > b ? a : b; }
 
 struct Layout {          // the single place that decides where things live in the workspace
-    size_t off_tab[3][2], off_tw[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
+    size_t off_tab[3][2], off_tw[3], off_tw2[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
     size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], total;
 };
 static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
@@ -60,6 +60,7 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
     for (int d = 0; d < 3; ++d) {
         for (int h = 0; h < 2; ++h) { Lo.off_tab[d][h] = o; o += align_up((size_t)g[d] * esz / 2); }
         Lo.off_tw[d] = o; o += align_up((size_t)g[d] * esz);
+        Lo.off_tw2[d] = o; o += align_up((size_t)g[d] * esz);
         Lo.off_k2[d] = o; o += align_up((size_t)g[d] * sizeof(double));
     }
     Lo.off_cA = o; o += align_up((size_t)(Ns + 1) * sizeof(double));
@@ -412,7 +413,7 @@ static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     March2Args A; std::memset(&A, 0, sizeof A);
     for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; A.e4[b] = c->e4[b]; }
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; }
-    A.tw = c->dim[0].tw;
+    A.tw = c->dim[0].tw2;
     A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nprop = c->nprop; A.nsteps = nsteps; A.lag = c->v2_lag; A.skew = c->v2_skew;
     A.qslot[0] = A.qslot[1] = 0;
     A.cnt = c->counters; A.ticket = (unsigned*)((char*)c->counters + c->counters_bytes - 256);
@@ -638,6 +639,27 @@ static double simpson_weight(int j, int a, int b) {     // composite Simpson 1/3
     return ((j - a) & 1) ? 4.0 / 3.0 : 2.0 / 3.0;
 }
 
+template <class T, int N, int EPT>
+static void fill_tw2_shape(std::vector<cplx<T>>& tw2) {
+    typedef Pencil<T, N, EPT> P; typedef PencilShape<N, EPT> S;
+    if (S::ONE) return;
+    for (int s = 0; s < P::TW2_SLOTS; ++s)
+        for (int k1 = 0; k1 < S::R1; ++k1) {
+            const long double a = 2.0L * kPiL * P::tw2_turns(s, k1);
+            tw2[s * S::R1 + k1] = mk<T>((T)std::cos(a), (T)std::sin(a));
+        }
+}
+template <class T>
+static void fill_tw2(int N, std::vector<cplx<T>>& tw2) {
+    switch (N) {
+        case 32: fill_tw2_shape<T, 32, 8>(tw2); break;
+        case 64: fill_tw2_shape<T, 64, 8>(tw2); break;
+        case 128: fill_tw2_shape<T, 128, 16>(tw2); break;
+        case 256: fill_tw2_shape<T, 256, 16>(tw2); break;
+        default: break;
+    }
+}
+
 // S1: everything that is computed once per simulation
 template <class T>
 static fts_status build_tables(Ctx* c) {
@@ -661,6 +683,9 @@ static fts_status build_tables(Ctx* c) {
         CK(cudaMemcpy(c->dim[d].tab[0], t0.data(), N * sizeof(T), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].tab[1], t1.data(), N * sizeof(T), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].tw, tw.data(), N * sizeof(cplx<T>), cudaMemcpyHostToDevice));
+        std::vector<cplx<T>> tw2(N, mk<T>(1, 0));              // twisted second stage of the FMA transform (fts_pencil.h, fwd2_b)
+        fill_tw2<T>(N, tw2);
+        CK(cudaMemcpy(c->dim[d].tw2, tw2.data(), N * sizeof(cplx<T>), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].k2, k2.data(), N * sizeof(double), cudaMemcpyHostToDevice));
     }
     std::vector<double> wA(c->Ns + 1), wB(c->Ns + 1);
@@ -715,7 +740,7 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
     c->ws = (char*)ws; c->ws_bytes = ws_bytes;
     for (int d = 0; d < 3; ++d) {
         c->dim[d].tab[0] = c->ws + Lo.off_tab[d][0]; c->dim[d].tab[1] = c->ws + Lo.off_tab[d][1];
-        c->dim[d].tw = c->ws + Lo.off_tw[d]; c->dim[d].k2 = (double*)(c->ws + Lo.off_k2[d]);
+        c->dim[d].tw = c->ws + Lo.off_tw[d]; c->dim[d].tw2 = c->ws + Lo.off_tw2[d]; c->dim[d].k2 = (double*)(c->ws + Lo.off_k2[d]);
     }
     c->cA = (double*)(c->ws + Lo.off_cA); c->cB = (double*)(c->ws + Lo.off_cB);
     c->scal = (double*)(c->ws + Lo.off_scal); c->kacc = (double*)(c->ws + Lo.off_kacc); c->partial = (double2*)(c->ws + Lo.off_partial);

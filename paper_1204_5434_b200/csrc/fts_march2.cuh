@@ -46,7 +46,7 @@ struct March2Maps {
 struct March2Args {
     void* F[2]; void* H[2]; const void* e4[2];
     const void* tab[3][2];       // per dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
-    const void* tw;              // inter-stage twiddles, per-(register, thread) layout
+    const void* tw;              // twiddles of the twisted second stage, tw2[slot * R1 + k1] (fts_pencil.h)
     int Ns, jA, nspecies, nprop, nsteps, lag, skew;
     int qslot[2];                // first slice index of propagator b inside its store (maps.x[M2_MAP_Q + b] covers the whole store)
     unsigned* ticket;
@@ -171,6 +171,9 @@ struct M2Sched {
 };
 
 
+__device__ __forceinline__ double flip_sign(double x) { return __hiloint2double(__double2hiint(x) ^ (int)0x80000000, __double2loint(x)); }
+__device__ __forceinline__ float flip_sign(float x) { return __int_as_float(__float_as_int(x) ^ (int)0x80000000); }
+
 // Per-thread view of a tile buffer: natural-layout access and the in-place diffusion (see the header).
 //   strided tile  (x, y passes): element (row rho, z) at  rho*RB + z*ES, 16-byte chunk index ^= (rho*RB >> 7) & SWM  (TMA swizzle)
 //   contiguous tile (z pass):    element i of pencil p at (p*N + i)*ES, no swizzle
@@ -194,9 +197,12 @@ struct M2Lane {
     static __device__ __forceinline__ C ld(const unsigned char* p) { return *reinterpret_cast<const C*>(p); }
     static __device__ __forceinline__ void st(unsigned char* p, C v) { *reinterpret_cast<C*>(p) = v; }
 
+    // Loads are issued in the order the first butterfly level consumes them (pairs r, r + 8), so that the butterflies start
+    // after two loads instead of nine.
+    template <int G> static constexpr int ld_order(int i) { return G == 1 ? ((i & 1) ? i / 2 + 8 : i / 2) : (i / 8 + 2 * ((i % 8) / 2) + 8 * (i & 1)); }
     template <bool CONTIG> __device__ __forceinline__ void load_nat(C (&v)[16], const unsigned char* base) const {
         const unsigned char* p = base + (CONTIG ? offc + VAc : offs + VAs);
-        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(p + r * TPP * stride<CONTIG>()); });
+        static_for<0, 16>([&](auto rr) { constexpr int r = ld_order<1>(decltype(rr)::value); v[r] = ld(p + r * TPP * stride<CONTIG>()); });
     }
     template <bool CONTIG> __device__ __forceinline__ void store_nat(const C (&v)[16], unsigned char* base) const {
         unsigned char* p = base + (CONTIG ? offc + VAc : offs + VAs);
@@ -219,7 +225,7 @@ struct M2Lane {
     }
     template <bool CONTIG> __device__ __forceinline__ void xld_b(C (&v)[16], const unsigned char* base) const {
         const unsigned vb = CONTIG ? VBc : VBs; base += CONTIG ? offc : offs;
-        static_for<0, 16>([&](auto rr) { constexpr int r = decltype(rr)::value; v[r] = ld(base + (vb ^ KB<CONTIG>(r))); });
+        static_for<0, 16>([&](auto rr) { constexpr int r = ld_order<G2>(decltype(rr)::value); v[r] = ld(base + (vb ^ KB<CONTIG>(r))); });
     }
     // exp(a ds d^2/dx_d^2) along the pencil = F^-1 [table] F, with the inverse transform run as conj o F o conj, so that ONE
     // forward-transform body (radix-R1 butterflies, twiddles, exchange A -> B, radix-R2 butterflies) is executed twice in a
@@ -230,18 +236,18 @@ struct M2Lane {
     __device__ __forceinline__ void diffuse(C (&v)[16], unsigned char* base, bool contig, const T* tab) const {
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
-            P::fwd_a(v, t, s_tw);
+            P::fwd2_a(v);
             __syncwarp();                                  // every lane has consumed what the buffer held / its B-pattern loads
             if (contig) xst_a<true>(v, base); else xst_a<false>(v, base);
             __syncwarp();
             if (contig) xld_b<true>(v, base); else xld_b<false>(v, base);
-            P::fwd_b(v);
+            P::fwd2_b(v, t, s_tw);
             if (pass == 0) {
 #pragma unroll
                 for (int r = 0; r < 16; ++r) { const T w = tab[t + TPP * r]; v[r] = mk<T>(v[r].x * w, v[r].y * (-w)); }
             } else {
 #pragma unroll
-                for (int r = 0; r < 16; ++r) v[r].y = -v[r].y;
+                for (int r = 0; r < 16; ++r) v[r].y = flip_sign(v[r].y);      // integer pipe: the fp64 pipe is the bound
             }
         }
         __syncwarp();                                      // all exchange reads done before anyone writes natural positions
@@ -270,7 +276,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
     M2Desc* s_desc = reinterpret_cast<M2Desc*>(b_iempty + M2_RING);  // [4]
 
     const int tid = threadIdx.x;
-    for (int i = tid; i < N; i += M2_LAUNCH) s_tw[i] = static_cast<const C*>(A.tw)[i];
+    for (int i = tid; i < N; i += M2_LAUNCH) s_tw[i] = static_cast<const C*>(A.tw)[i];      // tw2 layout (Pencil::fwd2_b), N/2 entries used
     for (int i = tid; i < 6 * N; i += M2_LAUNCH) s_tab[i] = static_cast<const T*>(A.tab[i / (2 * N)][(i / N) & 1])[i % N];
     if (tid == 0) {
         for (int i = 0; i < M2_NBUF; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_out[i], M2_NT); mbar_init(&b_free[i], 1); }

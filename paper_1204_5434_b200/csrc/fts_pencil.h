@@ -120,6 +120,113 @@ FTS_HD void dft_reg(cplx<T> (&v)[NV]) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// "Twisted" radix-2 DIF transform with FMA butterflies (used by the TMA march, fts_march2.cuh).
+//
+//   X[k] = sum_n x[n] (zeta w^k)^n,  w = exp(-2 pi i / R),  n, k = 0..R-1          (zeta = 1: the plain DFT)
+//
+// Splitting n = n' + (R/2) b gives  u = x[n'] + zeta^(R/2) x[n'+R/2]  (even k, same zeta) and
+// d = x[n'] - zeta^(R/2) x[n'+R/2]  (odd k, zeta' = zeta w), so EVERY butterfly has the form a +- W c with one W per
+// block: at level L (block size Rc = R / 2^(L-1)) block number blk uses  W = zeta^(Rc/2) * exp(-2 pi i E / 2^L),
+// E = bitrev(blk, L-1) < 2^(L-1).  The inter-stage twiddle of the two-stage pencil transform (zeta = exp(-2 pi i k1/N))
+// is thereby folded into the second stage's butterflies: no separate complex multiplies, and per level only
+// max(1, 2^(L-2)) distinct W are loaded (E >= 2^(L-2) is the same W times -i, an operand swap).
+// Cost per butterfly: 4 FMA for a + W c and 2 FMA for a - W c = 2a - (a + W c)  (6 fp64 instructions instead of the
+// 4 + 4 of "multiply, then add and subtract"); trivial W (1, -i) cost 4 adds; (+-1 -+ i)/sqrt2 costs 2 adds + 4 FMA.
+// A 128-point transform (16 x 8) needs 18.25 fp64 instructions per point instead of 23.5, a 256-point one 21.25
+// instead of 27.  Output X[k] is left at position bitrev(k) and renamed to natural order at compile time.
+// ------------------------------------------------------------------------------------------------
+template <class T> FTS_HD cplx<T> cmadd(cplx<T> a, cplx<T> w, cplx<T> c) {          // a + w c
+    if constexpr (sizeof(T) == 8) {
+#if defined(__CUDA_ARCH__)
+        return mk<T>(fma(-w.y, c.y, fma(w.x, c.x, a.x)), fma(w.y, c.x, fma(w.x, c.y, a.y)));
+#else
+        return a + w * c;
+#endif
+    } else return a + w * c;
+}
+template <class T> FTS_HD cplx<T> cmadd_mi(cplx<T> a, cplx<T> w, cplx<T> c) {       // a + (-i w) c
+    if constexpr (sizeof(T) == 8) {
+#if defined(__CUDA_ARCH__)
+        return mk<T>(fma(w.x, c.y, fma(w.y, c.x, a.x)), fma(-w.x, c.x, fma(w.y, c.y, a.y)));
+#else
+        const cplx<T> p = w * c; return mk<T>(a.x + p.y, a.y - p.x);
+#endif
+    } else { const cplx<T> p = w * c; return a + mk<T>(p.y, -p.x); }
+}
+// (a, c) <- (a + W c, a - W c), W = (MI ? -i : 1) * w
+template <bool MI, class T> FTS_HD void bfly_w(cplx<T>& a, cplx<T>& c, cplx<T> w) {
+    if constexpr (sizeof(T) == 8) {
+        const cplx<T> s = MI ? cmadd_mi(a, w, c) : cmadd(a, w, c);
+#if defined(__CUDA_ARCH__)
+        c = mk<T>(fma((T)2, a.x, -s.x), fma((T)2, a.y, -s.y));
+#else
+        c = mk<T>((T)2 * a.x - s.x, (T)2 * a.y - s.y);
+#endif
+        a = s;
+    } else {                                               // complex64: packed pair instructions, 4 per butterfly
+        cplx<T> p = w * c;
+        if (MI) p = mk<T>(p.y, -p.x);
+        c = a - p; a = a + p;
+    }
+}
+// (a, c) <- (a + W c, a - W c), W = exp(-2 pi i M / 16), M = 0..7 at compile time
+template <int M, class T> FTS_HD void bfly_c(cplx<T>& a, cplx<T>& c) {
+    static_assert(M >= 0 && M < 8, "constant twiddle out of range");
+    if constexpr (M == 0) { const cplx<T> s = a + c; c = a - c; a = s; }
+    else if constexpr (M == 4) { const cplx<T> p = mk<T>(c.y, -c.x); c = a - p; a = a + p; }
+    else if constexpr ((M == 2 || M == 6) && sizeof(T) == 8) {      // h (t1, t2) resp. h (t2, -t1), t1 = c.x + c.y, t2 = c.y - c.x
+        constexpr T h = (T)0.70710678118654752440;
+        const T t1 = c.x + c.y, t2 = c.y - c.x;
+        const T px = M == 2 ? t1 : t2, py = M == 2 ? t2 : -t1;
+#if defined(__CUDA_ARCH__)
+        c = mk<T>(fma(-h, px, a.x), fma(-h, py, a.y));
+        a = mk<T>(fma(h, px, a.x), fma(h, py, a.y));
+#else
+        c = mk<T>(a.x - h * px, a.y - h * py); a = mk<T>(a.x + h * px, a.y + h * py);
+#endif
+    } else bfly_w<false>(a, c, mk<T>((T)cos16(M), (T)(-sin16(M))));
+}
+
+// multiply by exp(-2 pi i M / 16), M = 0..3 at compile time (general position: 2 mul + 2 fma; M = 2: 2 add + 2 mul)
+template <int M, class T> FTS_HD cplx<T> mul_c16(cplx<T> a) {
+    if constexpr (M == 0) return a;
+    else return mul_w16<M, -1>(a);
+}
+template <class T> FTS_HD cplx<T> csq(cplx<T> a) { return mk<T>((a.x - a.y) * (a.x + a.y), (T)2 * a.x * a.y); }
+
+// In-register twisted DFT of R points held at v[OFF + S*i].  TWISTED: zp[j] = zeta^(2^j), j = 0..log2(R)-1, for this thread
+// and group; level L uses W = zp[log2(R) - L] * exp(-2 pi i (E mod 2^(L-2)) / 2^L) (the constant factor is a 16th root of
+// unity applied in registers: shared-memory bandwidth, not the fp64 pipe, bounds the passes, and a 16-byte twiddle load
+// costs four wavefronts however many lanes share it).  Otherwise zeta = 1 and every W is known at compile time.
+template <int R, int S, int OFF, bool TWISTED, class T, int NV, int NZ>
+FTS_HD void tdft_reg(cplx<T> (&v)[NV], const cplx<T> (&zp)[NZ]) {
+    if constexpr (R > 1) {
+        static_for<1, ilog2(R) + 1>([&](auto ll) {
+            constexpr int L = decltype(ll)::value, Rc = R >> (L - 1), half = Rc / 2, Q = L >= 2 ? (1 << (L - 2)) : 1;
+            static_for<0, (1 << (L - 1))>([&](auto bb) {
+                constexpr int blk = decltype(bb)::value, E = bitrev(blk, L - 1);
+                constexpr bool MI = L >= 2 && E >= Q;
+                if constexpr (TWISTED) {
+                    const cplx<T> w = mul_c16<((E % Q) * 16) / (1 << L)>(zp[ilog2(R) - L]);
+                    static_for<0, half>([&](auto ii) {
+                        constexpr int p0 = OFF + S * (blk * Rc + decltype(ii)::value), p1 = p0 + S * half;
+                        bfly_w<MI>(v[p0], v[p1], w);
+                    });
+                } else {
+                    static_for<0, half>([&](auto ii) {
+                        constexpr int p0 = OFF + S * (blk * Rc + decltype(ii)::value), p1 = p0 + S * half;
+                        bfly_c<(E * 16) / (1 << L)>(v[p0], v[p1]);
+                    });
+                }
+            });
+        });
+        cplx<T> tmp[R];
+        static_for<0, R>([&](auto ii) { constexpr int i = decltype(ii)::value; tmp[i] = v[OFF + S * bitrev(i, ilog2(R))]; });
+        static_for<0, R>([&](auto ii) { constexpr int i = decltype(ii)::value; v[OFF + S * i] = tmp[i]; });
+    }
+}
+
 // Factorisation of a pencil of N points over threads holding EPT values each.
 template <int N, int EPT>
 struct PencilShape {
@@ -179,6 +286,33 @@ struct Pencil {
             });
         }
     }
+    // Forward transform with FMA butterflies (see tdft_reg): part A = plain R1-point DFT per thread, no inter-stage
+    // multiply; part B (after the same exchange A -> B) = R2-point DFTs twisted by zeta = exp(-2 pi i k1 / N),
+    // k1 = t + TPP*g2.  Two twiddles are loaded per group, tw2[k1] = zeta and tw2[R1 + k1] = zeta^TW2_E1 (correctly rounded
+    // host values); the other powers zeta^(2^j) are one squaring away.
+    static constexpr int LOG2R2 = S::ONE ? 0 : ilog2(S::R2);
+    static constexpr int TW2_E1 = S::ONE ? 1 : (S::R2 >= 8 ? S::R2 / 4 : (S::R2 >= 4 ? S::R2 / 2 : 1));
+    static FTS_HD void fwd2_a(C (&v)[EPT]) {
+        const C one[1] = {mk<T>(1, 0)};
+        static_for<0, S::G1>([&](auto g) { tdft_reg<S::R1, S::G1, decltype(g)::value, false>(v, one); });
+    }
+    template <class TW>
+    static FTS_HD void fwd2_b(C (&v)[EPT], int t, const TW* tw2) {
+        if constexpr (!S::ONE)
+            static_for<0, S::G2>([&](auto g) {
+                constexpr int g2 = decltype(g)::value, J1 = ilog2(TW2_E1);
+                C zp[LOG2R2 > 0 ? LOG2R2 : 1];
+                const TW a = tw2[t + S::TPP * g2];
+                zp[0] = mk<T>((T)a.x, (T)a.y);
+                if constexpr (J1 > 0 && J1 < LOG2R2) { const TW b = tw2[S::R1 + t + S::TPP * g2]; zp[J1] = mk<T>((T)b.x, (T)b.y); }
+                static_for<1, LOG2R2>([&](auto jj) { constexpr int j = decltype(jj)::value; if constexpr (j != J1) zp[j] = csq(zp[j - 1]); });
+                tdft_reg<S::R2, S::G2, g2, true>(v, zp);
+            });
+    }
+    // host: angle (in units of 2 pi) of tw2[slot * R1 + k1], slot = 0, 1
+    static long double tw2_turns(int slot, int k1) { return -((long double)k1 * (slot ? TW2_E1 : 1) / (long double)N); }
+    static constexpr int TW2_SLOTS = S::ONE ? 0 : 2;
+
     // forward transform, part A: radix-R1 butterflies + inter-stage twiddle.
     template <class TW>
     static FTS_HD void fwd_a(C (&v)[EPT], int t, const TW* tw) {
