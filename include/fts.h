@@ -56,11 +56,12 @@ typedef struct {
     double fA, chiN, B, C;              /* block fraction, Flory parameter, excluded volume, chain density        */
     double lambda_plus, lambda_minus;   /* mobilities of Eq. 9 (Edwards uses lambda_plus); 0 is read as 1        */
     double noise_scale;                 /* multiplies eta in fts_cl_step: 1 = physical, 0 = deterministic         */
-    int    store_both;                  /* reserved: this version always keeps every q and q+ slice in HBM        */
+    int    store_both;                  /* 0: meet-in-the-middle store, slices 0..Ns/2 and the last one of q and of q+ are kept
+                                           (half the memory); 1: every slice is kept (needed for Pi)          */
 } fts_params;
 
-/* Bytes of device workspace fts_create needs: fields, Boltzmann factors, the contour-slice store
- * ((Ns+1) slices per propagator; PAPER.md:183 memory analysis), scratch, tables. */
+/* Bytes of device workspace fts_create needs: fields, Boltzmann factors, the contour-slice store (Ns/2 + 2 slices per
+ * propagator, or Ns + 1 with store_both; PAPER.md:183 memory analysis), density sums, scratch, tables. */
 fts_status fts_workspace_bytes(const int grid[3], int Ns, const fts_params* params, fts_precision prec, size_t* bytes);
 
 /* Builds the k-tables exp(-k_d^2 ds), exp(-k_d^2 ds/2) (once per simulation), the FFT
@@ -73,17 +74,24 @@ fts_status fts_destroy(fts_ctx* ctx);
 fts_status fts_set_fields(fts_ctx* ctx, const void* f0_dev, const void* f1_dev, void* stream);
 fts_status fts_get_fields(fts_ctx* ctx, void* f0_dev, void* f1_dev, void* stream);
 
-/* PAPER.md:143 Boltzmann factors, then Ns RQM4 steps (Eq. 12) of q and, batched with it, q+ (diblock);
- * every slice is written to the HBM store; Q = mean_x q(x,1) (Eq. 4) is left on the device.  Asynchronous. */
+/* PAPER.md:143 Boltzmann factors, then Ns RQM4 steps (Eq. 12) of q and, batched with it, q+ (diblock).  The march writes
+ * the retained slices to the HBM store and accumulates the Simpson density sums of Eq. 8 as it goes: from the middle of
+ * the chain on, each new slice is multiplied with the stored slice of the other propagator (meet-in-the-middle), so the
+ * product is never written and no second pass over the store is needed.  Q = mean_x q(x,1) (Eq. 4) is left on the
+ * device.  Asynchronous.  If the march gives up on an internal dependency (a bug or a lost SM; 5 s of wall clock) it stops,
+ * Q becomes NaN and the next call that returns host scalars reports FTS_ECUDA; fts_set_fields clears that state. */
 fts_status fts_propagate(fts_ctx* ctx, void* stream);
 /* March only the first nsteps contour steps (truncated parity at 256^3); Q is then mean_x q_nsteps. */
 fts_status fts_propagate_steps(fts_ctx* ctx, int nsteps, void* stream);
 
 /* phi_A (and phi_B) = (ds/Q) sum_j c_j q_j q+_{Ns-j}, composite Simpson per block (Eq. 8; plain bilinear
- * product).  Writes phi to caller memory, returns Q; synchronises `stream`.  phiB_dev NULL for one species. */
+ * product): normalises the sums the march accumulated.  Writes phi to caller memory, returns Q; synchronises
+ * `stream`.  phiB_dev NULL for one species.  FTS_ESTATE before a full fts_propagate. */
 fts_status fts_density_operators(fts_ctx* ctx, void* phiA_dev, void* phiB_dev, double Q_out[2], void* stream);
 
-/* Copy slice j of q (which = 0) or q+ (which = 1; q+ is indexed from the far chain end) to out_dev. */
+/* Copy slice j of q (which = 0) or q+ (which = 1; q+ is indexed from the far chain end) to out_dev.  Retained slices:
+ * j <= Ns/2 and the last slice of the march (q(r,1) after a full march); all of them with store_both = 1.
+ * FTS_ESTATE for a slice that was not retained or not reached. */
 fts_status fts_get_slice(fts_ctx* ctx, int which, int j, void* out_dev, void* stream);
 
 /* One SCFT iteration for the diblock melt (PAPER.md:84 forces; Eq. 11 at zero noise): W+ ascends with the
@@ -99,7 +107,8 @@ fts_status fts_cl_step(fts_ctx* ctx, double dt, int scheme, uint64_t seed, uint6
 
 /* Operators of the current fields; needs a completed fts_propagate.  H: Eq. 2 (Edwards, extensive) or
  * Eq. 3 / (CV) (diblock); mu = ln C - ln Q; Pi: volume derivative of ln Z at fixed lattice fields (derived in
- * DESIGN.md, not printed in the paper: secondary output).  Any pointer may be NULL.  Synchronises `stream`. */
+ * DESIGN.md, not printed in the paper: secondary output; needs store_both = 1, FTS_ESTATE otherwise).  Any pointer may be
+ * NULL.  Synchronises `stream`. */
 fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], void* stream);
 
 /* Tuning options (integers), effective from the next fts_propagate / step call; the library reads NO environment

@@ -73,8 +73,8 @@ def _p(t):
     return None if t is None else C.c_void_p(t.data_ptr())
 
 
-def make_params(model, fA=0.5, chiN=10.0, B=1.0, Cc=1.0, lambda_plus=1.0, lambda_minus=1.0, noise_scale=1.0):
-    return FtsParams(MODELS.get(model, model), fA, chiN, B, Cc, lambda_plus, lambda_minus, noise_scale, 1)
+def make_params(model, fA=0.5, chiN=10.0, B=1.0, Cc=1.0, lambda_plus=1.0, lambda_minus=1.0, noise_scale=1.0, store_both=0):
+    return FtsParams(MODELS.get(model, model), fA, chiN, B, Cc, lambda_plus, lambda_minus, noise_scale, int(store_both))
 
 
 def workspace_bytes(grid, Ns, params, precision="f64"):

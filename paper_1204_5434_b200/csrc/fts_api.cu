@@ -28,8 +28,9 @@ struct Ctx {
     // workspace carve-up
     DimTables dim[3];
     double *cA, *cB, *scal, *kacc; double2* partial;
-    void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2];
-    bool have_fields, have_prop; int marched;
+    void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2], *acc[2][2];
+    int keep, nslots;             // slice store: slices 0..keep at slot s, the last slice of a march at slot keep + 1 (fts_march.cuh)
+    bool have_fields, have_prop, have_phi; int marched;
     // march schedule (fts_march.cuh)
     Phase* phases;            // device: persistent template at [0], the four per-launch templates at [MARCH_MAXPH * (1..4)]
     unsigned* counters;       // device: completion counters, then ticket and error flag
@@ -51,9 +52,9 @@ static int counters_per_step(const int g[3]) { const int a = 2 + 2 * MARCH_MAXCH
 
 struct Layout {          // the single place that decides where things live in the workspace
     size_t off_tab[3][2], off_tw[3], off_tw2[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
-    size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], total;
+    size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], off_acc[2][2], total; int keep, nslots;
 };
-static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
+static Layout make_layout(const int g[3], int Ns, int model, size_t esz, int store_both) {
     Layout Lo; size_t o = 0;
     const size_t M = (size_t)g[0] * g[1] * g[2], field = align_up(M * esz);
     const int nprop = model == FTS_MODEL_DIBLOCK ? 2 : 1;
@@ -77,7 +78,13 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz) {
     for (int i = 0; i < 2; ++i) { Lo.off_H[i] = o; o += (i < nprop) ? field : 0; }
     for (int i = 0; i < 2; ++i) { Lo.off_phi[i] = o; o += field; }
     for (int i = 0; i < 2; ++i) { Lo.off_G[i] = o; o += field; }
-    for (int i = 0; i < 2; ++i) { Lo.off_q[i] = o; o += (i < nprop) ? align_up((size_t)(Ns + 1) * M * esz) : 0; }   // contour-slice store
+    for (int b = 0; b < 2; ++b)
+        for (int a = 0; a < 2; ++a) { Lo.off_acc[b][a] = o; o += (b < nprop && a < nprop) ? field : 0; }      // density sums [propagator][species]
+    // contour-slice store: meet-in-the-middle keeps slices 0..Ns/2 and the last one per propagator,
+    // store_both keeps all Ns + 1 (needed for Pi)
+    Lo.keep = store_both ? Ns : Ns / 2;
+    Lo.nslots = store_both ? Ns + 1 : Ns / 2 + 2;
+    for (int i = 0; i < 2; ++i) { Lo.off_q[i] = o; o += (i < nprop) ? align_up((size_t)Lo.nslots * M * esz) : 0; }
     Lo.total = o;
     return Lo;
 }
@@ -164,11 +171,11 @@ static Job mkjob(const void* in, void* out, int op) { Job j; j.in = in; j.out = 
 static int ew_blocks(size_t M) { size_t b = (M + 255) / 256; return (int)(b < 148 * 16 ? b : 148 * 16); }
 
 template <class T, int OP>
-static cudaError_t reduce(const Ctx* c, const void* a, const void* b, double p, double scale, double* out_dev, cudaStream_t st) {
+static cudaError_t reduce(const Ctx* c, const void* a, const void* b, double p, double scale, double* out_dev, cudaStream_t st, const int* poison = nullptr) {
     const int M = (int)c->M;
     int nb = (M + RED_THREADS - 1) / RED_THREADS; if (nb > RED_BLOCKS) nb = RED_BLOCKS;
     reduce_partial_kernel<T, OP><<<nb, RED_THREADS, 0, st>>>((const cplx<T>*)a, (const cplx<T>*)b, M, p, c->partial);
-    reduce_final_kernel<OP><<<1, 1024, 0, st>>>(c->partial, nb, scale, out_dev);
+    reduce_final_kernel<OP><<<1, 1024, 0, st>>>(c->partial, nb, scale, out_dev, poison);
     g_launches += 2;
     return cudaGetLastError();
 }
@@ -275,6 +282,13 @@ static std::vector<Phase> make_template(int nprop, int nchunks, int lag, bool in
     return v;
 }
 
+static DensArgs dens_args(const Ctx* c, int nsteps) {
+    DensArgs D;
+    for (int b = 0; b < 2; ++b) for (int a = 0; a < 2; ++a) D.acc[b][a] = c->acc[b][a];
+    D.cA = c->cA; D.cB = c->cB; D.on = nsteps == c->Ns; D.keep = c->keep; D.half = c->Ns / 2;
+    return D;
+}
+
 template <class T>
 static void fill_march_args(const Ctx* c, MarchArgs& A, int nsteps) {
     std::memset(&A, 0, sizeof A);
@@ -282,6 +296,7 @@ static void fill_march_args(const Ctx* c, MarchArgs& A, int nsteps) {
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; A.tw[d] = c->dim[d].tw; A.g[d] = c->g[d]; }
     A.M = (long long)c->M; A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nsteps = nsteps;
     A.done = c->counters; A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
+    A.dens = dens_args(c, nsteps);
 }
 
 // Decide the schedule once per context (needs the device: occupancy, SM count) and upload the templates.
@@ -318,7 +333,10 @@ static fts_status plan_march(Ctx* c) {
     // per-launch templates (stream-ordered mode): kind k at all[MARCH_MAXPH*(1+k)], one phase per propagator
     int cl[4]; phase_counts(c, mi[0], mi[1], mi[2], tz, Nx, cl);
     for (int k = 0; k < 4; ++k)
-        for (int b = 0; b < c->nprop; ++b) all[MARCH_MAXPH * (1 + k) + b] = mkphase(b * cl[k], k, b, 0, 0);
+        for (int b = 0; b < c->nprop; ++b) {
+            all[MARCH_MAXPH * (1 + k) + b] = mkphase(b * cl[k], k, b, 0, 0);
+            all[MARCH_MAXPH * (1 + k) + 2 + b] = mkphase(0, k, b, 0, 0);       // propagator b alone (see march_t)
+        }
     if (!c->persistent) for (int k = 0; k < 4; ++k) c->cnt[k] = cl[k];
     CK(cudaMemcpy(c->phases, all.data(), all.size() * sizeof(Phase), cudaMemcpyHostToDevice));
     return FTS_OK;
@@ -383,7 +401,7 @@ static fts_status plan_march2(Ctx* c) {
     for (int b = 0; b < 2 && ok; ++b) {
         const int pb = b < c->nprop ? b : 0;
         ok = ok && make_tile_map(c, &c->maps.x[M2_MAP_F + b], c->F[pb], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_H + b], c->H[pb], 1, true) &&
-             make_tile_map(c, &c->maps.x[M2_MAP_E + b], c->e4[b], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_Q + b], c->q[pb], c->Ns + 1, true) &&
+             make_tile_map(c, &c->maps.x[M2_MAP_E + b], c->e4[b], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_Q + b], c->q[pb], c->nslots, true) &&
              make_tile_map(c, &c->maps.y[0 + b], c->F[pb], 1, false) && make_tile_map(c, &c->maps.y[2 + b], c->H[pb], 1, false);
     }
     if (!ok) {
@@ -415,7 +433,8 @@ static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; }
     A.tw = c->dim[0].tw2;
     A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nprop = c->nprop; A.nsteps = nsteps; A.lag = c->v2_lag; A.skew = c->v2_skew;
-    A.qslot[0] = A.qslot[1] = 0;
+    for (int b = 0; b < 2; ++b) A.q[b] = c->q[b < c->nprop ? b : 0];
+    A.dens = dens_args(c, nsteps);
     A.cnt = c->counters; A.ticket = (unsigned*)((char*)c->counters + c->counters_bytes - 256);
     A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
     long long grid = (long long)c->v2_occ * c->sms;
@@ -429,6 +448,8 @@ template <class T>
 static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     MarchArgs A; fill_march_args<T>(c, A, nsteps);
     CK(cudaMemsetAsync(c->counters, 0, c->counters_bytes - 128, st));          // counters and ticket; the error flag stays until fts_set_fields
+    if (nsteps == c->Ns)                                                        // S6: the density sums the T items accumulate into
+        for (int b = 0; b < c->nprop; ++b) for (int a = 0; a < c->nspecies; ++a) CK(cudaMemsetAsync(c->acc[b][a], 0, c->M * c->esz, st));
     if (c->v2) return march2_t<T>(c, nsteps, st);
     if (c->persistent) {
         A.nchunks = c->nchunks; A.planes = c->planes;
@@ -453,8 +474,17 @@ static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     for (int j = 0; j <= nsteps; ++j) {
         for (int k = 0; k < 4; ++k) {
             if (k != PH_T && j == nsteps) break;
-            A.phases = c->phases + MARCH_MAXPH * (1 + k); A.nphases = c->nprop; A.tickets_per_round = c->nprop * c->cnt[k];
             A.round0 = A.round1 = j;
+            if (k == PH_T && c->nprop == 2 && A.dens.on && j == A.dens.half) {
+                // the middle of the chain: q+'s item multiplies q+_h with the slice q_h that q's item of the SAME step stores
+                // (DensArgs), so the two propagators' T phases cannot share a launch here
+                for (int b = 0; b < 2; ++b) {
+                    A.phases = c->phases + MARCH_MAXPH * (1 + k) + 2 + b; A.nphases = 1; A.tickets_per_round = c->cnt[k];
+                    CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
+                }
+                continue;
+            }
+            A.phases = c->phases + MARCH_MAXPH * (1 + k); A.nphases = c->nprop; A.tickets_per_round = c->nprop * c->cnt[k];
             CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
         }
     }
@@ -470,17 +500,22 @@ static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
     CK(cudaGetLastError());
     fts_status rc = march_t<T>(c, nsteps, st); if (rc) return rc;
     // S7 (Eq. 4): Q = (1/M) sum_x q_Ns(x), fixed-order tree
-    CK((reduce<T, RED_SUM>(c, (const cplx<T>*)c->q[0] + (size_t)nsteps * M, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st)));
-    c->marched = nsteps; c->have_prop = true;
+    // (a march that gave up on a dependency leaves its error flag set: Q then becomes NaN, so that everything downstream of it --
+    // densities, field updates, operators -- is visibly invalid, and every call that returns scalars reports FTS_ECUDA)
+    CK((reduce<T, RED_SUM>(c, (const cplx<T>*)c->q[0] + (size_t)slice_slot(nsteps, c->keep) * M, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st,
+                           (const int*)((const char*)c->counters + c->counters_bytes - 128))));
+    c->marched = nsteps; c->have_prop = true; c->have_phi = false;
     return FTS_OK;
 }
 
+// S6, last step (Eq. 8): phi = (ds / Q) (sums of q's items + sums of q+'s items); the sums were accumulated by
+// the march's T items.  Written to phiA / phiB (the context's own phi fields or the caller's).
 template <class T>
 static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
-    const cplx<T>* q = (const cplx<T>*)c->q[0];
-    const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];              // homopolymer: q+ == q
-    density_kernel<T><<<(unsigned)((c->M + 255) / 256), 256, 0, st>>>(q, qd, c->M, c->Ns, c->cA, c->cB, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA,
-                                                                       c->nspecies == 2 ? (cplx<T>*)phiB : nullptr);
+    const bool two = c->nprop == 2;
+    density_finish_kernel<T><<<ew_blocks(c->M), 256, 0, st>>>((const cplx<T>*)c->acc[0][0], two ? (const cplx<T>*)c->acc[1][0] : nullptr,
+                                                             two ? (const cplx<T>*)c->acc[0][1] : nullptr, two ? (const cplx<T>*)c->acc[1][1] : nullptr,
+                                                             (int)c->M, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA, two ? (cplx<T>*)phiB : nullptr);
     g_launches += 1;
     CK(cudaGetLastError());
     return FTS_OK;
@@ -586,6 +621,7 @@ static fts_status operators_t(Ctx* c, double* Ho, double* muo, double* Pio, cuda
     const cplx<T>* q = (const cplx<T>*)c->q[0];
     const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];
     fts_status rc;
+    if (Pio && c->keep != Ns) { c->err = "Pi needs every slice of q and q+: create the context with store_both = 1"; return FTS_ESTATE; }
     if (Pio) {                                             // K_j = (1/M) sum_x q+_{Ns-j} Laplacian(q_j)
         Filt f; f.type = FILT_NEGK2; f.a = 1.0; f.b = f.c = 0.0;
         for (int j = 0; j <= Ns; ++j) {
@@ -718,7 +754,7 @@ const char* fts_last_error(const fts_ctx* c) { return c ? c->err.c_str() : "null
 fts_status fts_workspace_bytes(const int grid[3], int Ns, const fts_params* P, fts_precision prec, size_t* bytes) {
     if (!bytes) return FTS_EINVAL;
     fts_status rc = validate(grid, nullptr, Ns, P, prec); if (rc) return rc;
-    *bytes = make_layout(grid, Ns, P->model, prec == FTS_F64 ? 16 : 8).total;
+    *bytes = make_layout(grid, Ns, P->model, prec == FTS_F64 ? 16 : 8, P->store_both).total;
     return FTS_OK;
 }
 
@@ -726,7 +762,7 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
     if (!cell || !out || !ws) return FTS_EINVAL;
     fts_status rc = validate(grid, cell, Ns, P, prec); if (rc) return rc;
     const size_t esz = prec == FTS_F64 ? 16 : 8;
-    const Layout Lo = make_layout(grid, Ns, P->model, esz);
+    const Layout Lo = make_layout(grid, Ns, P->model, esz, P->store_both);
     if (ws_bytes < Lo.total || ((uintptr_t)ws & 255)) return FTS_EWORKSPACE;
     fts_ctx* c = new (std::nothrow) fts_ctx;
     if (!c) return FTS_EINVAL;
@@ -748,9 +784,11 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
     for (int i = 0; i < 2; ++i) {
         c->e4[i] = c->ws + Lo.off_e4[i]; c->F[i] = c->ws + Lo.off_F[i]; c->H[i] = c->ws + Lo.off_H[i];
         c->q[i] = c->ws + Lo.off_q[i]; c->phi[i] = c->ws + Lo.off_phi[i]; c->G[i] = c->ws + Lo.off_G[i];
+        for (int a = 0; a < 2; ++a) c->acc[i][a] = c->ws + Lo.off_acc[i][a];
     }
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
-    c->have_fields = c->have_prop = false; c->marched = 0; c->occ = 0;
+    c->keep = Lo.keep; c->nslots = Lo.nslots;
+    c->have_fields = c->have_prop = c->have_phi = false; c->marched = 0; c->occ = 0;
     c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
@@ -787,6 +825,7 @@ fts_status fts_set_fields(fts_ctx* c, const void* f0, const void* f1, void* stre
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaMemcpyAsync(c->f0, f0, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
     if (c->P.model == FTS_MODEL_DIBLOCK) CK(cudaMemcpyAsync(c->f1, f1, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync((char*)c->counters + c->counters_bytes - 128, 0, sizeof(int), st));      // new fields: clear a previous march's error flag
     c->have_fields = true; c->have_prop = false;
     return FTS_OK;
 }
@@ -822,8 +861,9 @@ fts_status fts_density_operators(fts_ctx* c, void* phiA, void* phiB, double Q_ou
 fts_status fts_get_slice(fts_ctx* c, int which, int j, void* out, void* stream) {
     if (!c || !out || which < 0 || which > 1 || j < 0 || j > c->Ns) return FTS_EINVAL;
     if (!c->have_prop || j > c->marched) return FTS_ESTATE;
+    if (j > c->keep && j != c->marched) { c->err = "slice not retained by the meet-in-the-middle store (store_both = 0)"; return FTS_ESTATE; }
     const char* base = (const char*)c->q[which == 1 ? c->nprop - 1 : 0];
-    CK(cudaMemcpyAsync(out, base + (size_t)j * c->M * c->esz, c->M * c->esz, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    CK(cudaMemcpyAsync(out, base + (size_t)slice_slot(j, c->keep) * c->M * c->esz, c->M * c->esz, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return FTS_OK;
 }
 

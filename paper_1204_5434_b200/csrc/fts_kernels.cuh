@@ -5,7 +5,7 @@
 //                   field-update filters — forward, 3-D multiplier, inverse.  Used by the SCFT / Eq. 11 updates and Pi.
 // boltzmann_kernel  exp(-w ds/4) per species.
 // reduce_kernel     deterministic two-level sums / max (Q of Eq. 4, H of Eq. 2-3, residuals).
-// density_kernel    Simpson contour sums of q_j q+_{Ns-j} (Eq. 8).
+// density_finish    phi = (ds/Q) x the Simpson sums the march accumulated (Eq. 8).
 // update kernels    forces of PAPER.md:84, Euler-Maruyama / semi-implicit updates of Eq. 9-11, Philox noise.
 #ifndef FTS_KERNELS_CUH
 #define FTS_KERNELS_CUH
@@ -214,7 +214,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partial_kernel(const cplx<
     if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
 }
 template <int OP>
-__global__ void __launch_bounds__(1024) reduce_final_kernel(const double2* partial, int n, double scale, double* out) {
+__global__ void __launch_bounds__(1024) reduce_final_kernel(const double2* partial, int n, double scale, double* out, const int* poison) {
     __shared__ double2 sm[1024];
     sm[threadIdx.x] = threadIdx.x < n ? partial[threadIdx.x] : make_double2(0.0, 0.0);
     __syncthreads();
@@ -222,29 +222,31 @@ __global__ void __launch_bounds__(1024) reduce_final_kernel(const double2* parti
         if (threadIdx.x < s) sm[threadIdx.x] = red_comb<OP>(sm[threadIdx.x], sm[threadIdx.x + s]);
         __syncthreads();
     }
-    if (threadIdx.x == 0) { out[0] = sm[0].x * scale; out[1] = sm[0].y * scale; }
+    if (threadIdx.x == 0) {
+        const bool bad = poison && *poison != 0;           // the march gave up on a dependency: make the result visibly invalid
+        out[0] = bad ? __longlong_as_double(0x7ff8000000000000ll) : sm[0].x * scale;
+        out[1] = bad ? __longlong_as_double(0x7ff8000000000000ll) : sm[0].y * scale;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
-// S6 density (Eq. 8): phi_A = (ds/Q) sum_j cA_j q_j q+_{Ns-j}, phi_B likewise; fp64 accumulators
+// S6 density (Eq. 8): the Simpson sums  sum_j c_j q_j q+_{Ns-j}  are accumulated inside the march by the T
+// items (fts_march.cuh DensArgs: meet-in-the-middle, one sum per propagator and species); this kernel adds the two
+// propagators' sums and multiplies by ds / Q.
 // ------------------------------------------------------------------------------------------------
 template <class T>
-__global__ void __launch_bounds__(256) density_kernel(const cplx<T>* q, const cplx<T>* qd, size_t M, int Ns, const double* cA, const double* cB,
-                                                      const double* Qdev, double ds, cplx<T>* phiA, cplx<T>* phiB) {
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= M) return;
-    double ax = 0, ay = 0, bx = 0, by = 0;
-#pragma unroll 4
-    for (int j = 0; j <= Ns; ++j) {
-        const cplx<T> u = q[(size_t)j * M + i], w = qd[(size_t)(Ns - j) * M + i];
-        const double px = (double)u.x * (double)w.x - (double)u.y * (double)w.y, py = (double)u.x * (double)w.y + (double)u.y * (double)w.x;
-        const double wa = cA[j], wb = cB[j];
-        ax += wa * px; ay += wa * py;
-        bx += wb * px; by += wb * py;
-    }
+__global__ void density_finish_kernel(const cplx<T>* a0, const cplx<T>* a1, const cplx<T>* b0, const cplx<T>* b1, int M, const double* Qdev, double ds,
+                                      cplx<T>* phiA, cplx<T>* phiB) {
     const double qx = Qdev[0], qy = Qdev[1], den = ds / (qx * qx + qy * qy);     // multiply by ds * conj(Q)/|Q|^2
-    phiA[i] = mk<T>((T)((ax * qx + ay * qy) * den), (T)((ay * qx - ax * qy) * den));
-    if (phiB) phiB[i] = mk<T>((T)((bx * qx + by * qy) * den), (T)((by * qx - bx * qy) * den));
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        double ax = (double)a0[i].x, ay = (double)a0[i].y;
+        if (a1) { ax += (double)a1[i].x; ay += (double)a1[i].y; }
+        phiA[i] = mk<T>((T)((ax * qx + ay * qy) * den), (T)((ay * qx - ax * qy) * den));
+        if (phiB) {
+            const double bx = (double)b0[i].x + (double)b1[i].x, by = (double)b0[i].y + (double)b1[i].y;
+            phiB[i] = mk<T>((T)((bx * qx + by * qy) * den), (T)((by * qx - bx * qy) * den));
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -42,6 +42,22 @@ struct Phase {              // one entry of the round template ("round" j holds 
     signed char prop_off;   // bit 0: propagator b; bit 1: the phase belongs to step (round - 1)
 };
 
+// Slice store and density accumulation, shared by both march kernels.  Slices s <= keep and the last slice of the march
+// are retained (slot s, resp. keep + 1); store_both keeps every slice (keep = Ns).  With h = Ns/2 the T item that emits
+//   q_j   (j > h)   adds  c_j     q_j  q+_{Ns-j}  (stored, Ns-j < h)   into acc[0][species],
+//   q+_m  (m >= h)  adds  c_{Ns-m} q+_m q_{Ns-m}  (stored, Ns-m <= h)  into acc[1][species],
+// so every pair (j, Ns-j) is visited exactly once and the product is never written.  One propagator (q+ = q): the item of
+// q_j, j >= h, adds (c_j + c_{Ns-j}) q_j q_{Ns-j} for j > h and c_h q_h^2 for j = h.  acc is zeroed before the march;
+// phi = (ds/Q) (acc[0] + acc[1]) is formed afterwards (density_finish_kernel).
+struct DensArgs {
+    void* acc[2][2];            // [propagator][species], un-normalised sums; element type = the field type
+    const double* cA; const double* cB;     // Simpson weights per contour index (0 outside the block)
+    int on;                     // accumulate (full marches only)
+    int keep;                   // slices 0..keep are retained at slot s; the last slice of the march at slot keep + 1
+    int half;                   // h = Ns / 2
+};
+__host__ __device__ inline int slice_slot(int s, int keep) { return s <= keep ? s : keep + 1; }
+
 struct MarchArgs {
     void* q[2]; void* F[2]; void* H[2]; const void* e4[2];
     const void* tab[3][2];      // per dimension: exp(-k_d^2 ds)/N_d, exp(-k_d^2 ds/2)/N_d
@@ -55,6 +71,8 @@ struct MarchArgs {
     unsigned* ticket;           // NULL: one item per CTA (ticket = blockIdx.x) and no dependency waits (stream order)
     unsigned* done;             // completion counters [prop][step][2 + 2*nchunks]: T, Y2 (all slabs), Y1[slab], Z[slab]
     int* err;                   // set to 1 if a dependency wait timed out
+    // S6 (Eq. 8): Simpson density sums accumulated by the T items, meet-in-the-middle
+    DensArgs dens;
 };
 
 template <class T> struct vec2;
@@ -76,6 +94,7 @@ __device__ __forceinline__ unsigned ld_relaxed(const unsigned* p) {
     return v;
 }
 __device__ __forceinline__ void fence_acquire() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 
 template <class T, int N, int EPT, int TZ>
 struct MarchCfg {
@@ -111,13 +130,20 @@ __device__ __forceinline__ bool mbar_test(uint64_t* b, unsigned parity) {
                  : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ bool mbar_wait(uint64_t* b, unsigned parity) {      // false: gave up (never hang the GPU)
+// A wait inside a CTA (descriptor hand-off) can only fail through a bug: it traps after 20 s of wall clock (the launch then
+// fails loudly with a CUDA error) instead of hanging the GPU or leaving a barrier half-arrived.
+__device__ __forceinline__ bool mbar_wait(uint64_t* b, unsigned parity) {
     unsigned ok, tries = 0;
-    do {
+    unsigned long long t0 = 0;
+    for (;;) {
         asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                      : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
-    } while (!ok && ++tries < (1u << 24));
-    return ok != 0;
+        if (ok) return true;
+        if ((++tries & 4095u) == 0) {
+            unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+            if (t0 == 0) t0 = t; else if (t - t0 > 20000000000ull) __trap();
+        }
+    }
 }
 
 // exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform.
@@ -210,7 +236,20 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
             if (ph.kind == PH_Z) { need = (unsigned)A.nY1; return cnt + 2 + ph.chunk; }
             need = (unsigned)A.nZ; return cnt + 2 + A.nchunks + ph.chunk;
         };
-        unsigned issued = 0, completed = 0, spins = 0;
+        // T items that accumulate densities also read a slice the OTHER propagator (or, with one propagator, an earlier step)
+        // stored: its T phase must be complete.  It lies at least a step back in ticket order, so this never waits in practice.
+        auto dependency2 = [&](const Phase& ph, int s, unsigned& need) -> const unsigned* {
+            need = 0;
+            if (ph.kind != PH_T || !A.dens.on) return nullptr;
+            const int b = ph.prop_off & 1, nprop = A.nspecies == 2 ? 2 : 1;      // diblock: two propagators
+            if (nprop == 2 ? (b == 0 ? s <= A.dens.half : s < A.dens.half) : s <= A.dens.half) return nullptr;
+            need = (unsigned)A.ntT;
+            return A.done + ((size_t)(nprop == 2 ? 1 - b : 0) * (A.Ns + 1) + (A.Ns - s)) * C2;
+        };
+        unsigned issued = 0, completed = 0;
+        unsigned long long t_wait0 = 0; unsigned spins = 0;
+        bool aborted = false;
+        const unsigned* pw2 = nullptr; unsigned pneed2 = 0;
         unsigned tk_pending = A.ticket ? atomicAdd(A.ticket, 1u) : blockIdx.x;       // drawn one item ahead
         bool have = false, exhausted = false;
         int ps = 0, plo = 0, pidx = 0;                 // the item waiting for its dependency
@@ -252,13 +291,27 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
                     const bool live = ph.kind == PH_T ? (ps >= 0 && ps <= A.nsteps) : (ps >= 0 && ps < A.nsteps);
                     if (!live) continue;               // ticket of a phase outside the march: no work
                     pw = A.ticket ? dependency(ph, ps, pneed) : nullptr;
-                    have = true; spins = 0;
+                    pw2 = A.ticket ? dependency2(ph, ps, pneed2) : nullptr;
+                    have = true; spins = 0; t_wait0 = 0;
                 }
-                bool ok = !pw || pw == dep_ok;
+                bool ok = (!pw || pw == dep_ok) && !pw2;
                 if (!ok) {
-                    ok = ld_relaxed(pw) >= pneed;
-                    if (!ok && ++spins > (1u << 22)) { atomicExch(A.err, 1); ok = true; }      // never hang the GPU: flag it and carry on
+                    ok = (!pw || pw == dep_ok || ld_relaxed(pw) >= pneed) && (!pw2 || ld_relaxed(pw2) >= pneed2);
+                    if (!ok && (++spins & 1023u) == 0) {
+                        // another CTA's work is 5 s late (wall clock): a bug or a lost CTA.  Flag it and DRAIN: no further item is
+                        // released, the compute warps get the end sentinel, Q is poisoned by the reduction (never compute on).
+                        const unsigned long long now = globaltimer_ns();
+                        if (t_wait0 == 0) t_wait0 = now;
+                        else if (now - t_wait0 > 5000000000ull) { atomicExch(A.err, 1); aborted = true; }
+                    }
                     if (ok) fence_acquire();
+                }
+                if (aborted) {
+                    const int slot = issued % R;
+                    s_item[slot][3] = 0;
+                    mbar_arrive(&s_full[slot]);
+                    exhausted = true; have = false;
+                    continue;
                 }
                 if (ok) {
                     if (pw) dep_ok = pw;
@@ -381,7 +434,17 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
             Coords<T> c; coords(slot, c);
             const bool start = c.s < A.nsteps;
             const int sp_now = species(c.b, c.s), sp_prev = species(c.b, c.s - 1);
-            C* qs = static_cast<C*>(A.q[c.b]) + (long long)c.s * A.M;
+            const bool keep = c.s <= A.dens.keep || c.s == A.nsteps;
+            C* qs = static_cast<C*>(A.q[c.b]) + (long long)slice_slot(c.s, A.dens.keep) * A.M;
+            // density pair of this slice (DensArgs): partner slice and Simpson weights
+            const bool two = A.nspecies == 2;
+            const int h = A.dens.half, jp = (two && c.b == 1) ? A.Ns - c.s : c.s;      // contour index j of the pair (j, Ns - j)
+            const bool dens = A.dens.on && (two ? (c.b == 0 ? c.s > h : c.s >= h) : c.s >= h);
+            const bool self = !two && c.s == h;
+            const C* partner = static_cast<const C*>(A.q[two ? 1 - c.b : 0]) + (long long)(A.Ns - c.s) * A.M;      // stored: Ns - s <= keep
+            double wA = 0.0, wB = 0.0;
+            if (dens) { wA = A.dens.cA[jp]; wB = A.dens.cB[jp]; if (!two && !self) wA += A.dens.cA[A.Ns - jp]; }
+            C* accA = static_cast<C*>(A.dens.acc[c.b][0]); C* accB = static_cast<C*>(A.dens.acc[c.b][1]);
             const C* e4s = static_cast<const C*>(A.e4[sp_now]);
             const bool reload = !combine || sp_now != sp_prev;
 #pragma unroll
@@ -394,7 +457,12 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
                     const C h = v[r] * e;
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                 }
-                if (c.active) stcg(qs + i, v[r]);                     // the slice store IS the step's output write
+                if (c.active && keep) stcg(qs + i, v[r]);             // the slice store IS the step's output write
+                if (dens && c.active) {                               // Eq. 8: this slice times the stored partner, weighted, into the sums
+                    const C pr = v[r] * (self ? v[r] : ldcg(partner + i));
+                    if (wA != 0.0) { const C a = ldcg(accA + i); stcg(accA + i, mk<T>(a.x + (T)wA * pr.x, a.y + (T)wA * pr.y)); }
+                    if (wB != 0.0) { const C a = ldcg(accB + i); stcg(accB + i, mk<T>(a.x + (T)wB * pr.x, a.y + (T)wB * pr.y)); }
+                }
                 if (start) {
                     if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
                     const C hb = v[r] * e;

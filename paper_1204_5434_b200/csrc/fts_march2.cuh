@@ -35,7 +35,7 @@
 namespace fts {
 
 enum { M2_NBUF = 3, M2_RING = 4, M2_NT = 128, M2_LAUNCH = 192 };
-enum { M2_FIRST = 1, M2_FIN = 2, M2_START = 4, M2_RELOAD = 8, M2_JOBH = 16 };
+enum { M2_FIRST = 1, M2_FIN = 2, M2_START = 4, M2_RELOAD = 8, M2_JOBH = 16, M2_KEEP = 32, M2_DENS = 64 };
 enum { M2_MAP_F = 0, M2_MAP_H = 2, M2_MAP_E = 4, M2_MAP_Q = 6 };     // + propagator (F, H, Q) or species (E)
 
 struct March2Maps {
@@ -48,7 +48,8 @@ struct March2Args {
     const void* tab[3][2];       // per dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
     const void* tw;              // twiddles of the twisted second stage, tw2[slot * R1 + k1] (fts_pencil.h)
     int Ns, jA, nspecies, nprop, nsteps, lag, skew;
-    int qslot[2];                // first slice index of propagator b inside its store (maps.x[M2_MAP_Q + b] covers the whole store)
+    const void* q[2];            // slice stores (the density partner is read straight from global memory)
+    DensArgs dens;               // S6: Simpson density sums accumulated by the T items (fts_march.cuh)
     unsigned* ticket;
     unsigned* cnt;               // completion counters [prop][step][2 + 2 N]: T, Y2 (all planes), Y1[plane], Z[plane]
     int* err;
@@ -321,6 +322,33 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
 #ifdef FTS_M2_NODEPS
                 dep = nullptr;                                             // measurement build only: wrong results, shows what the schedule costs
 #endif
+                // T items that accumulate densities read a slice stored by the other propagator's T phase of step Ns - s (one
+                // propagator: its own); that phase lies at least a step back in ticket order
+                const unsigned* dep2 = nullptr;
+                if (d.kind == PH_T && A.dens.on) {
+                    const bool two = A.nprop == 2;
+                    if (two ? (d.b == 0 ? d.s > A.dens.half : d.s >= A.dens.half) : d.s >= A.dens.half) {
+                        d.flags |= M2_DENS;
+                        if (!(!two && d.s == A.dens.half)) dep2 = A.cnt + ((size_t)(two ? 1 - d.b : 0) * (A.Ns + 1) + (A.Ns - d.s)) * Cfg::C2;
+                    }
+                }
+                if (d.kind == PH_T && (d.s <= A.dens.keep || d.s == A.nsteps)) d.flags |= M2_KEEP;
+#ifdef FTS_M2_NODEPS
+                dep2 = nullptr;
+#endif
+                if (dep2) {
+                    unsigned spins = 0;
+                    unsigned long long t0 = 0;
+                    while (ld_relaxed(dep2) < (unsigned)Cfg::NT_X) {
+                        if ((++spins & 4095u) == 0) {
+                            const unsigned long long t = m2_now_ns();
+                            if (t0 == 0) t0 = t; else if (t - t0 > 5000000000ull) { aborted = true; break; }
+                        }
+                        __nanosleep(20);
+                    }
+                    if (aborted) { atomicExch(A.err, 1); break; }
+                    if (!dep || dep == dep_ok) fence_acquire();
+                }
                 if (dep && dep != dep_ok) {
                     unsigned spins = 0;
                     unsigned long long t0 = 0;
@@ -399,9 +427,10 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                 bool store = true;
                 if (d.kind == PH_T) {
                     if (k > 0 && !(d.flags & M2_START)) store = false;
+                    if (k == 0 && !(d.flags & M2_KEEP)) store = false;            // meet-in-the-middle: this slice is not retained
                     if (store) {
                         const CUtensorMap* mp = &maps.x[k == 0 ? M2_MAP_Q + d.b : (k == 1 ? M2_MAP_F + d.b : M2_MAP_H + d.b)];
-                        const int c3 = k == 0 ? A.qslot[d.b] + d.s : 0;
+                        const int c3 = k == 0 ? slice_slot(d.s, A.dens.keep) : 0;
                         for (int g = 0; g < Cfg::G; ++g) { int c0, c1; xcoord(d.idx, g, c0, c1); m2_tma_store4(mp, c0, c1, 0, c3, src + g * Cfg::TILEB); }
                     }
                 } else if (d.kind == PH_Z) {
@@ -472,11 +501,25 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
             const bool fin = flags & M2_FIN, start = flags & M2_START, reload = flags & M2_RELOAD;
             const unsigned char* pe = pB + sub + VAs; const unsigned char* pf = pC + sub + VAs;
             unsigned char* pq = pA + sub + VAs; unsigned char* ph = pC + sub + VAs;
+            const bool dens = flags & M2_DENS;
             const C* e4s = nullptr; int gbase = 0;
-            if (reload) {                                               // block junction: the new species' factors straight from global memory
+            if (reload || dens) {                                       // element r of this thread inside a field: gbase + r TPP N^2
                 const int idx = dv->idx;
                 const int tile = idx * Cfg::G + w / Cfg::WPT, z = (tile % (N / 8)) * 8 + (w % Cfg::WPT) * Cfg::ZPW + zz, iy = tile / (N / 8);
-                e4s = static_cast<const C*>(A.e4[dv->spS]); gbase = (t * N + iy) * N + z;
+                gbase = (t * N + iy) * N + z;
+            }
+            if (reload) e4s = static_cast<const C*>(A.e4[dv->spS]);     // block junction: the new species' factors straight from global memory
+            // S6 (Eq. 8, DensArgs): this slice times the stored partner slice, Simpson-weighted, into the sums
+            const C* partner = nullptr; C* accA = nullptr; C* accB = nullptr; T wA = 0, wB = 0; bool self = false;
+            if (dens) {
+                const int b = dv->b, s = dv->s; const bool two = A.nprop == 2;
+                const int jp = (two && b == 1) ? A.Ns - s : s;
+                self = !two && s == A.dens.half;
+                double a = A.dens.cA[jp]; const double bb = A.dens.cB[jp];
+                if (!two && !self) a += A.dens.cA[A.Ns - jp];
+                wA = (T)a; wB = (T)bb;
+                partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N;
+                accA = static_cast<C*>(A.dens.acc[b][0]); accB = static_cast<C*>(A.dens.acc[b][1]);
             }
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
@@ -487,6 +530,12 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                 } else v[r] = mk<T>(1, 0);                              // q(x,0) = 1, q+(x,s=1) = 1
                 L.st(pq + r * TPP * RB, v[r]);
+                if (dens) {
+                    const int gi = gbase + r * TPP * N * N;
+                    const C pr = v[r] * (self ? v[r] : ldcg(partner + gi));
+                    if (wA != (T)0) { const C a = ldcg(accA + gi); stcg(accA + gi, mk<T>(a.x + wA * pr.x, a.y + wA * pr.y)); }
+                    if (wB != (T)0) { const C a = ldcg(accB + gi); stcg(accB + gi, mk<T>(a.x + wB * pr.x, a.y + wB * pr.y)); }
+                }
                 if (start) {
                     if (reload) e = ldcg(e4s + gbase + r * TPP * N * N);
                     const C hb = v[r] * e;

@@ -28,10 +28,11 @@ def _kw(cfg):
     return dict(fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
 
 
-def _pair(B, oracle, cfg, precision="f64", **extra):
+def _pair(B, oracle, cfg, precision="f64", store_both=1, **extra):
+    """store_both = 1 (every slice kept) unless the test is about the default meet-in-the-middle store."""
     kw = _kw(cfg); kw.update(extra)
     dt = torch.complex128 if precision == "f64" else torch.complex64
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **kw)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=store_both, **kw)
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **kw)    # the fp64 oracle judges both precisions
     f1 = None if cfg.f1 is None else _dev(cfg.f1, dt)
     g.set_fields(_dev(cfg.f0, dt), f1)
@@ -108,7 +109,7 @@ def test_uniform_field_and_invariants_on_device(B):
     Q, phi, _ = g.density_operators()
     assert abs(Q - np.exp(-w0)) < 1e-13 and float((phi - 1).abs().max()) < 1e-12
     cfg = inputs.small_diblock(grid=(32, 32, 32), Ns=20, fA=0.4)
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", **_kw(cfg))
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", store_both=1, **_kw(cfg))
     g.set_fields(_dev(cfg.f0), _dev(cfg.f1))
     g.propagate()
     Q, pa, pb = g.density_operators()
@@ -256,7 +257,7 @@ def test_tma_march_equals_ticket_march_128(B, precision, model, nsteps):
         kw = {}
     outs = []
     for mode in (2, 3):
-        g = B.Fts((128,) * 3, (9.0, 10.0, 11.0), Ns, model, precision=precision, options={"march": mode}, **kw)
+        g = B.Fts((128,) * 3, (9.0, 10.0, 11.0), Ns, model, precision=precision, options={"march": mode}, store_both=1, **kw)
         g.set_fields(*[torch.from_numpy(np.ascontiguousarray(f)).to("cuda:0").to(g.cdtype) for f in fields])
         g.propagate(nsteps)
         sl = [g.get_slice(w, j).clone() for w in ((0, 1) if model == "diblock" else (0,)) for j in range(nsteps + 1)]
@@ -300,7 +301,7 @@ def test_full_size_config5(B, oracle, n, nsteps, precision):
     a truncated march (the oracle needs ~10 s per 256^3 step), then properties that hold at any size on the full march."""
     cfg = inputs.config5(n)
     dt = torch.complex128 if precision == "f64" else torch.complex64
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=1, **_kw(cfg))
     g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
     g.propagate(nsteps)
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
@@ -329,7 +330,7 @@ def test_full_size_config5(B, oracle, n, nsteps, precision):
 def _developed_solve_parity(B, oracle, cfg, precision="f64", tolQ=1e-11, tolphi=1e-9, operators=False):
     f0, f1 = inputs.developed(cfg)
     dt = torch.complex128 if precision == "f64" else torch.complex64
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=1 if operators else 0, **_kw(cfg))
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
     g.set_fields(_dev(f0, dt), None if f1 is None else _dev(f1, dt))
     o.set_fields(f0, f1)
@@ -437,7 +438,7 @@ def test_march_soak_bit_identical(B, n, precision, reps):
     claimed dynamically by ~300-450 CTAs) must be bit-identical every time; a race would show as a differing bit."""
     cfg = inputs.small_diblock(grid=(n, n, n), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
     dt = torch.complex128 if precision == "f64" else torch.complex64
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", precision=precision, **_kw(cfg))
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", precision=precision, store_both=n % 64 == 0, **_kw(cfg))      # both store layouts
     g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
     g.propagate()
     Q0, pa0, pb0 = g.density_operators()
@@ -450,3 +451,59 @@ def test_march_soak_bit_identical(B, n, precision, reps):
         Q, pa, pb = g.density_operators()
         assert Q == Q0 and torch.equal(pa, pa0) and torch.equal(pb, pb0), rep
         assert torch.equal(g.get_slice(1, cfg.Ns), last), rep
+
+
+# ------------------------------------------------------------------------------------------------
+# S6: densities accumulated inside the march, meet-in-the-middle store (the default, store_both = 0)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("model,grid,Ns,fA", [("diblock", (16, 16, 16), 20, 0.3), ("diblock", (32, 32, 32), 10, 0.4), ("diblock", (16, 8, 32), 12, 0.5),
+                                               ("edwards", (16, 16, 16), 10, 0.5), ("external", (32, 32, 32), 6, 0.5), ("external", (8, 16, 8), 2, 0.5)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_meet_in_the_middle_store(B, oracle, model, grid, Ns, fA, precision):
+    """Default store: Q and phi as with the full store and as the oracle's plain sum over all slices (block junction left, right
+    and at the middle; one and two propagators; persistent and per-phase launches); retained slices 0..Ns/2 and Ns match the
+    oracle; any other slice is FTS_ESTATE; Pi (needs every slice) is FTS_ESTATE."""
+    if model == "diblock":
+        cfg = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=Ns, fA=fA)
+    elif model == "edwards":
+        cfg = inputs.config4(grid=grid, cell=(4.0, 4.0, 4.0), Ns=Ns)
+    else:
+        cfg = inputs.config1(grid=grid, cell=(4.0, 4.0, 4.0), Ns=Ns)
+    g, o = _pair(B, oracle, cfg, precision=precision, store_both=0)
+    two = model == "diblock"
+    if precision == "f64":
+        _cmp_solve(g, o, 1e-11, 1e-9, two)
+    else:
+        g.propagate(); o.propagate()
+        Qg, pa, pb = g.density_operators(); Qo, oa, ob = o.density_operators()
+        assert abs(Qg - Qo) < 2e-4 * abs(Qo) and np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 * max(1.0, np.max(np.abs(oa)))
+        if two:
+            assert np.max(np.abs(pb.cpu().numpy() - ob)) < 2e-4
+    tol = 1e-9 if precision == "f64" else 2e-4
+    for which in ((0, 1) if two else (0,)):
+        for j in (0, 1, Ns // 2, Ns):
+            assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - o.get_slice(which, j))) < tol, (which, j)
+        if Ns // 2 + 1 < Ns:
+            with pytest.raises(B.FtsError) as e:
+                g.get_slice(which, Ns // 2 + 1)
+            assert e.value.status == 2                 # FTS_ESTATE
+    with pytest.raises(B.FtsError) as e:
+        g.operators(want_pi=True)
+    assert e.value.status == 2
+    H, mu, _ = g.operators(want_pi=False)
+    Ho, muo, _ = o.operators()
+    assert abs(mu - muo) < (1e-10 if precision == "f64" else 2e-4) * max(1.0, abs(muo))
+    # a truncated march keeps its last slice (the slice Q is taken from) and leaves the densities undefined
+    k = Ns // 2 + 1 if Ns > 2 else 1
+    g.propagate(k); o.propagate(k)
+    assert np.max(np.abs(g.get_slice(0, k).cpu().numpy() - o.get_slice(0, k))) < tol
+    with pytest.raises(B.FtsError):
+        g.density_operators()
+
+
+def test_workspace_halves_with_the_default_store(B):
+    from paper_1204_5434_b200.binding import make_params, workspace_bytes
+    a = workspace_bytes((64, 64, 64), 100, make_params("diblock", fA=0.5, store_both=0))
+    b = workspace_bytes((64, 64, 64), 100, make_params("diblock", fA=0.5, store_both=1))
+    field = 64 ** 3 * 16
+    assert b - a == 2 * (101 - 52) * field            # Ns/2 + 2 slices per propagator instead of Ns + 1

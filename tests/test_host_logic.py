@@ -32,7 +32,9 @@ def test_library_exports_every_declared_symbol(libpath):
 def test_argument_validation_without_gpu(libpath):
     from paper_1204_5434_b200 import binding as B
     ok = B.make_params("diblock", fA=0.3, chiN=20.0)
-    assert B.workspace_bytes((32, 32, 32), 100, ok) > 2 * 101 * 32 ** 3 * 16          # holds both slice stores
+    assert B.workspace_bytes((32, 32, 32), 100, ok) > 2 * 52 * 32 ** 3 * 16           # meet-in-the-middle: Ns/2 + 2 slices per propagator
+    both = B.make_params("diblock", fA=0.3, chiN=20.0, store_both=1)
+    assert B.workspace_bytes((32, 32, 32), 100, both) > 2 * 101 * 32 ** 3 * 16        # store_both: every slice of q and q+
     assert B.workspace_bytes((32, 32, 32), 100, ok, "f32") < B.workspace_bytes((32, 32, 32), 100, ok)
     for grid, Ns, p, status in [((32, 32, 12), 100, ok, 6),                           # not a power of two
                                 ((512, 8, 8), 100, ok, 6),
