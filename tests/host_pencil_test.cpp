@@ -2,7 +2,8 @@
 // iteration, every __syncthreads() a phase boundary.  Checks, for each supported (N, EPT):
 //   forward result == O(N^2) DFT in the documented spectral layout k = t + TPP*r,
 //   forward -> inverse == N * identity, and the shared-memory exchange is bank-conflict-free for
-//   both CTA layouts the kernels use.  Not the oracle: this exercises product code on the CPU.
+//   both CTA layouts the kernels use; and the same for the twisted FMA transform of the TMA march.
+// Not the oracle: this exercises product code on the CPU.
 #include <cmath>
 #include <complex>
 #include <cstdio>
@@ -80,8 +81,46 @@ void run(int npencil, double tol) {
     if (!ok) ++failures;
 }
 
+// The twisted FMA transform of the TMA march (fwd2_a, exchange A -> B, fwd2_b with the two-slot twiddle table): forward result
+// == O(N^2) DFT in the same spectral layout; conj o forward o conj == N * inverse.
+template <class T, int N, int EPT>
+void run_twisted(double tol) {
+    typedef Pencil<T, N, EPT> P; typedef typename P::S S;
+    const int TPP = S::TPP;
+    const long double PI = 3.14159265358979323846264338327950288L;
+    std::vector<cplx<T>> tw2(2 * N + 2, mk<T>(1, 0));
+    for (int s = 0; s < P::TW2_SLOTS; ++s) for (int k1 = 0; k1 < S::R1; ++k1) { const long double a = 2 * PI * P::tw2_turns(s, k1); tw2[s * S::R1 + k1] = mk<T>((T)cosl(a), (T)sinl(a)); }
+    std::vector<cd> x(N);
+    srand(N * 7 + EPT);
+    for (auto& e : x) e = cd(rand() / (double)RAND_MAX - 0.5, rand() / (double)RAND_MAX - 0.5);
+    std::vector<cplx<T>> v((size_t)TPP * EPT), u((size_t)TPP * EPT);
+    auto fwd = [&]() {
+        for (int t = 0; t < TPP; ++t) P::fwd2_a(*reinterpret_cast<cplx<T>(*)[EPT]>(&v[(size_t)t * EPT]));
+        if (S::ONE) { u = v; return; }
+        for (int t = 0; t < TPP; ++t) for (int r = 0; r < EPT; ++r) { const int g2 = r % S::G2, n2 = r / S::G2; u[(size_t)t * EPT + r] = v[(size_t)n2 * EPT + t + TPP * g2]; }
+        for (int t = 0; t < TPP; ++t) P::fwd2_b(*reinterpret_cast<cplx<T>(*)[EPT]>(&u[(size_t)t * EPT]), t, tw2.data());
+    };
+    for (int t = 0; t < TPP; ++t) for (int r = 0; r < EPT; ++r) v[(size_t)t * EPT + r] = mk<T>((T)x[t + TPP * r].real(), (T)x[t + TPP * r].imag());
+    fwd();
+    double err = 0;
+    for (int k = 0; k < N; ++k) {
+        cd ref(0, 0);
+        for (int n = 0; n < N; ++n) ref += x[n] * std::polar(1.0, (double)(-2 * PI * ((long)k * n % N) / N));
+        err = std::max(err, std::abs(ref - cd(u[(size_t)(k % TPP) * EPT + k / TPP].x, u[(size_t)(k % TPP) * EPT + k / TPP].y)));
+    }
+    for (size_t i = 0; i < u.size(); ++i) v[i] = mk<T>(u[i].x, -u[i].y);      // conj o forward o conj
+    fwd();
+    double err2 = 0;
+    for (int n = 0; n < N; ++n) err2 = std::max(err2, std::abs(x[n] * (double)N - cd(u[(size_t)(n % TPP) * EPT + n / TPP].x, -u[(size_t)(n % TPP) * EPT + n / TPP].y)));
+    const bool ok = err < tol * N && err2 < tol * N * N;
+    printf("%s N=%3d EPT=%2d twisted FMA transform fwd_err=%.2e rt_err=%.2e %s\n", sizeof(T) == 8 ? "f64" : "f32", N, EPT, err, err2, ok ? "OK" : "FAIL");
+    if (!ok) ++failures;
+}
+
 template <class T>
 void all(double tol) {
+    run_twisted<T, 8, 8>(tol); run_twisted<T, 16, 16>(tol); run_twisted<T, 32, 8>(tol); run_twisted<T, 64, 8>(tol);
+    run_twisted<T, 64, 16>(tol); run_twisted<T, 128, 16>(tol); run_twisted<T, 256, 16>(tol);
     constexpr int TZ = 128 / (2 * sizeof(T));
     run<T, 8, 8, true>(TZ, tol);    run<T, 8, 8, false>(32, tol);
     run<T, 16, 16, true>(TZ, tol);  run<T, 16, 16, false>(32, tol);
