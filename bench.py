@@ -107,7 +107,7 @@ def oracle_sample(cfg, budget_s):
     from oracle import binding as ob
     M = int(np.prod(cfg.grid))
     nprop = 2 if cfg.model == "diblock" else 1
-    rate = _ORACLE_RATE.get(cfg.name, M / (4.5e-8 * M * math.log2(M)))      # first guess: ~18 s per RQM4 step at 256^3
+    rate = _ORACLE_RATE.get(cfg.name, 2.5e6)                                # first guess: the oracle's measured ~2.5e6 grid-pt·steps/s per core
     n = int(budget_s * rate / (M * nprop))
     if n >= 1:
         n = min(n, cfg.Ns)
@@ -130,6 +130,44 @@ def oracle_sample(cfg, budget_s):
     return units / dt, dt, what + ", cost linear in steps"
 
 
+def config_dict(cfg, kind, prec, world, extra=None):
+    """The same keys in both arms (the driver compares them)."""
+    d = {"workload": cfg.name, "grid": list(cfg.grid), "Ns": cfg.Ns, "kind": kind, "precision": prec,
+         "rqm4_steps_per_step": rqm4_steps_per_step(cfg, kind), "l2": "flushed between timed steps (256 MiB write)",
+         "parallelism": f"replicas x{world}" if world > 1 else "1 GPU"}
+    d.update(extra or {})
+    return d
+
+
+def oracle_host_aggregate(workload, budget_s, n_steps_hint):
+    """BASELINE.md plan (ii): P independent oracle processes concurrently on the host's cores (no threading inside the oracle);
+    P = the box's core count, capped by memory and at 32.  Returns (aggregate units/s, P, cpu_count, text)."""
+    import psutil
+    cfg, _ = make_workload(workload)
+    M = int(np.prod(cfg.grid))
+    per_proc = 16.0 * M * (14 + 2 * (n_steps_hint + 1))          # bytes: tables, fields, Boltzmann factors, temporaries, the slices of the sample
+    ncpu = os.cpu_count() or 1
+    P = max(1, min(ncpu, 32, int(0.5 * psutil.virtual_memory().available / per_proc)))
+    procs = [subprocess.Popen([sys.executable, os.path.abspath(__file__), "--oracle-worker", "--workload", workload, "--budget", str(budget_s)],
+                              stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True) for _ in range(P)]
+    t0 = time.perf_counter()
+    outs = [p.communicate()[0] for p in procs]
+    wall = time.perf_counter() - t0
+    units = 0.0
+    for o in outs:
+        try:
+            units += json.loads(o.strip().splitlines()[-1])["units"]
+        except Exception:
+            pass
+    return units / wall, P, ncpu, f"{P} concurrent oracle processes (host has {ncpu} cores), each the one-core sample; wall {wall:.1f} s incl. process start-up"
+
+
+def run_oracle_worker(args):
+    cfg, _ = make_workload(args.workload)
+    v, dt, what = oracle_sample(cfg, args.budget)
+    print(json.dumps({"units": v * dt, "seconds": dt}))
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the same workload/metric; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -148,8 +186,8 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * full_units / value, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": cfg.name, "grid": list(cfg.grid), "Ns": cfg.Ns, "kind": kind,
-                                         "note": "ms_per_step is the full step extrapolated from the sample"},
+        "data": "synthetic", "config": config_dict(cfg, kind, "f64", 1),
+        "note": "ms_per_step is the full step extrapolated from the bounded sample (the oracle's cost is linear in contour steps)",
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"per step: {what}"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -283,36 +321,41 @@ def run_gpu(args):
     f_alg, b_alg = 30.0 * M * math.log2(M), 3.0 * E * M        # per RQM4 step of one propagator
     t_fp, t_hbm = f_alg / (best * 1e12), b_alg / (pk["hbm_gbs"] * 1e9)
     t_step = ms_march * 1e-3 / rq
-    pass_launches = 1                                          # the whole march of one solve is ONE persistent launch (cubic grids)
-    traffic = None
+    pass_launches = max(1, march_launches - 3)                 # fts_propagate = boltzmann + march launch(es) + 2 reduction kernels; cubic grids: ONE persistent march launch
+    traffic, traffic_src = None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"{args.workload}_{prec}")
+        tj = json.load(open(tp))
+        traffic = tj.get(f"{args.workload}_{prec}")
+        traffic_src = {k: tj.get(k) for k in ("_note", "_commit", "_sm_mhz")}
     if t_fp >= t_hbm:
         roof = {"bound": "alu", "achieved": f_alg / t_step / 1e12, "peak": best, "unit": "TFLOP/s", "frac": t_fp / t_step,
                 "peak_kind": f"vector {prec} FMA chains measured in this run (nominal {FP64_NOMINAL_TFLOPS if prec == 'f64' else FP32_NOMINAL_TFLOPS:.1f})"}
     else:
         roof = {"bound": "hbm", "achieved": b_alg / t_step / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": t_hbm / t_step, "peak_kind": pk_kind}
-    roof.update({"traffic": traffic, "kernel": "march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve)", "launches_per_march": pass_launches,
+    roof.update({"traffic": traffic, "traffic_source": traffic_src, "kernel": "march2_kernel / march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve, densities accumulated in the T items)", "launches_per_march": pass_launches,
                  "avg_launch_us": ms_march * 1e3 / pass_launches, "alg_flops_per_launch": f_alg * rq / pass_launches,
                  "alg_bytes_per_launch": b_alg * rq / pass_launches, "march_ms": ms_march, "march_launches_all_kernels": march_launches,
                  "hbm_view": {"achieved_GBs_algorithmic": b_alg / t_step / 1e9, "peak_GBs": pk["hbm_gbs"], "peak_kind": pk_kind,
                               "frac_of_floor": t_hbm / t_step}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-           "config": {"workload": cfg.name, "model": None, "grid": list(cfg.grid), "Ns": cfg.Ns, "kind": kind, "precision": prec,
-                      "rqm4_steps_per_step": rqm4_steps_per_step(cfg, kind), "l2": "flushed between timed steps (256 MiB write)",
-                      "parallelism": f"replicas x{world}" if world > 1 else "1 GPU"},
+           "config": config_dict(cfg, kind, prec, world),
            "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
                                                                                       "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),
            "e2e": {"value": world * units * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": sum(h.numel() * h.element_size() for h in host),
                    "d2h_bytes_per_step": sum(b.numel() * b.element_size() for b in back[:1 if kind == 'propagate' else None])},
            "gpu_launches": launches, "roofline": roof}
-    del out["config"]["model"]
     if world == 1 and not args.no_cpu_baseline:
         v, dt, what = oracle_sample(cfg, 20.0)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what, "seconds": dt}
+        try:
+            n_hint = max(1, int(20.0 * v / (M * nprop)))
+            va, P, ncpu, text = oracle_host_aggregate(args.workload, 20.0, n_hint)
+            out["cpu_baseline"]["whole_host"] = {"value": va, "unit": UNIT, "cores": P, "host_cores": ncpu, "sample": text}
+        except Exception as e:                                   # the aggregate is context; never lose the bench line over it
+            out["cpu_baseline"]["whole_host"] = {"unavailable": repr(e)}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -328,8 +371,12 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="fts_set_option (tuning experiments), e.g. --opt march=2")
+    ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--budget", type=float, default=20.0, help=argparse.SUPPRESS)
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.oracle_worker:
+        run_oracle_worker(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_gpu(args)

@@ -10,8 +10,9 @@
  *
  * Units and conventions: lengths in Rg, contour s in [0,1], ds = 1/Ns; the diffusion
  * factor is exp(-k^2 ds).  Grids: shape (Nx,Ny,Nz), layout [ix][iy][iz] with z contiguous, interleaved
- * (re,im); FTS_F64 = complex128, FTS_F32 = complex64.  Every grid dimension must be a power of two in
- * [8, 256] (FTS_EUNSUPPORTED otherwise; the paper benchmarks power-of-two grids).
+ * (re,im); FTS_F64 = complex128, FTS_F32 = complex64.  Every grid dimension must be 1 or a power of two in
+ * [8, 256] (FTS_EUNSUPPORTED otherwise; the paper benchmarks power-of-two grids); dimensions of 1
+ * give the 1-D and 2-D problems of PAPER.md:193 (e.g. (N,1,1), (Nx,Ny,1)); 512 is not supported.
  *
  * Stored fields:  FTS_MODEL_EXTERNAL  f0 = w                       (one species in a given complex field)
  *                 FTS_MODEL_EDWARDS   f0 = Omega                   (chain feels i*Omega; Eq. 2)
@@ -44,7 +45,7 @@ typedef enum {
     FTS_EWORKSPACE = 3,    /* workspace smaller than fts_workspace_bytes, or not 256-byte aligned                   */
     FTS_ECUDA = 4,         /* a CUDA call failed; text in fts_last_error                                          */
     FTS_ENONFINITE = 5,    /* Q is NaN/Inf (diverged CL run)                                                       */
-    FTS_EUNSUPPORTED = 6   /* grid dimension not a power of two in [8,256]; model/step combination not defined    */
+    FTS_EUNSUPPORTED = 6   /* grid dimension not 1 or a power of two in [8,256]; model/step combination not defined */
 } fts_status;
 
 typedef enum { FTS_F64 = 0, FTS_F32 = 1 } fts_precision;

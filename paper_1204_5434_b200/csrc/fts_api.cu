@@ -89,8 +89,17 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz, int sto
     return Lo;
 }
 
-static int ept_of(int N) { return (N == 16 || N >= 128) ? 16 : 8; }     // must match the launch_*_n switches
-static bool pow2_ok(int n) { return n >= 8 && n <= 256 && (n & (n - 1)) == 0; }
+static int ept_of(int N) { return N == 1 ? 1 : ((N == 16 || N >= 128) ? 16 : 8); }     // must match the launch_*_n switches
+static bool pow2_ok(int n) { return n == 1 || (n >= 8 && n <= 256 && (n & (n - 1)) == 0); }
+
+// 1-D and 2-D problems (Fig. 1) are grids with dimensions of 1.  A dimension of 1 does not affect the
+// memory layout ([ix][iy][iz], z contiguous), so internally the ones are moved to the front: (N,1,1) -> (1,1,N),
+// (Nx,Ny,1) -> (1,Nx,Ny).  The kernels then see pencils of length 1 along x (and y) - the identity - and a real z.
+static void squeeze_grid(const int grid[3], const double* cell, int g[3], double L[3]) {
+    int n = 2;
+    for (int d = 2; d >= 0; --d) if (grid[d] != 1) { g[n] = grid[d]; L[n] = cell ? cell[d] : 1.0; --n; }
+    for (int d = 2; d >= 0 && n >= 0; --d) if (grid[d] == 1) { g[n] = 1; L[n] = cell ? cell[d] : 1.0; --n; }
+}
 
 static fts_status validate(const int grid[3], const double* cell, int Ns, const fts_params* P, int prec) {
     if (!grid || !P) return FTS_EINVAL;
@@ -107,6 +116,7 @@ static fts_status validate(const int grid[3], const double* cell, int Ns, const 
         if (!(P->chiN > 0)) return FTS_EINVAL;
     } else if (Ns & 1) return FTS_EINVAL;
     for (int d = 0; d < 3; ++d) if (!pow2_ok(grid[d])) return FTS_EUNSUPPORTED;
+    if (grid[0] == 1 && grid[1] == 1 && grid[2] == 1) return FTS_EUNSUPPORTED;
     return FTS_OK;
 }
 
@@ -136,6 +146,7 @@ static cudaError_t launch_pass_inst(const PassArgs& A, int njobs, cudaStream_t s
 template <class T, int TZ>
 static cudaError_t launch_pass_n(int N, const PassArgs& A, int njobs, cudaStream_t st) {
     switch (N) {
+        case 1: return launch_pass_inst<T, 1, 1, TZ>(A, njobs, st);
         case 8: return launch_pass_inst<T, 8, 8, TZ>(A, njobs, st);
         case 16: return launch_pass_inst<T, 16, 16, TZ>(A, njobs, st);
         case 32: return launch_pass_inst<T, 32, 8, TZ>(A, njobs, st);
@@ -209,6 +220,7 @@ static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, M
 template <class T, int TZ>
 static cudaError_t launch_march_n(int N, const MarchArgs& A, int grid, bool query, MarchInfo* info, int* occ, cudaStream_t st) {
     switch (N) {
+        case 1: return launch_march_inst<T, 1, 1, TZ>(A, grid, query, info, occ, st);
         case 8: return launch_march_inst<T, 8, 8, TZ>(A, grid, query, info, occ, st);
         case 16: return launch_march_inst<T, 16, 16, TZ>(A, grid, query, info, occ, st);
         case 32: return launch_march_inst<T, 32, 8, TZ>(A, grid, query, info, occ, st);
@@ -754,13 +766,17 @@ const char* fts_last_error(const fts_ctx* c) { return c ? c->err.c_str() : "null
 fts_status fts_workspace_bytes(const int grid[3], int Ns, const fts_params* P, fts_precision prec, size_t* bytes) {
     if (!bytes) return FTS_EINVAL;
     fts_status rc = validate(grid, nullptr, Ns, P, prec); if (rc) return rc;
-    *bytes = make_layout(grid, Ns, P->model, prec == FTS_F64 ? 16 : 8, P->store_both).total;
+    int g[3]; double L[3];
+    squeeze_grid(grid, nullptr, g, L);
+    *bytes = make_layout(g, Ns, P->model, prec == FTS_F64 ? 16 : 8, P->store_both).total;
     return FTS_OK;
 }
 
-fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts_params* P, fts_precision prec, void* ws, size_t ws_bytes, fts_ctx** out) {
-    if (!cell || !out || !ws) return FTS_EINVAL;
-    fts_status rc = validate(grid, cell, Ns, P, prec); if (rc) return rc;
+fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns, const fts_params* P, fts_precision prec, void* ws, size_t ws_bytes, fts_ctx** out) {
+    if (!cell_user || !out || !ws) return FTS_EINVAL;
+    fts_status rc = validate(grid_user, cell_user, Ns, P, prec); if (rc) return rc;
+    int grid[3]; double cell[3];
+    squeeze_grid(grid_user, cell_user, grid, cell);
     const size_t esz = prec == FTS_F64 ? 16 : 8;
     const Layout Lo = make_layout(grid, Ns, P->model, esz, P->store_both);
     if (ws_bytes < Lo.total || ((uintptr_t)ws & 255)) return FTS_EWORKSPACE;

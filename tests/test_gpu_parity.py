@@ -507,3 +507,30 @@ def test_workspace_halves_with_the_default_store(B):
     b = workspace_bytes((64, 64, 64), 100, make_params("diblock", fA=0.5, store_both=1))
     field = 64 ** 3 * 16
     assert b - a == 2 * (101 - 52) * field            # Ns/2 + 2 slices per propagator instead of Ns + 1
+
+
+# ------------------------------------------------------------------------------------------------
+# N3: 1-D and 2-D grids (Fig. 1) as grids with dimensions of 1
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("grid,cell", [((64, 1, 1), (5.0, 1.0, 1.0)), ((1, 1, 128), (1.0, 1.0, 7.0)), ((1, 256, 1), (2.0, 9.0, 1.0)),
+                                        ((32, 16, 1), (3.0, 4.0, 1.0)), ((1, 8, 64), (1.0, 3.0, 5.0)), ((128, 1, 8), (6.0, 1.0, 2.0))])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_one_and_two_dimensional_grids(B, oracle, grid, cell, precision):
+    """The same kernels with pencils of length 1 along the missing dimensions: propagator slices, Q, phi, one SCFT iteration
+    (3-D filter passes of length 1) and one CL step (scheme 1: the Eq. 11 filter) against the oracle on the same grid."""
+    cfg = inputs.small_diblock(grid=grid, cell=cell, Ns=12, fA=0.5, complex_fields=True)
+    g, o = _pair(B, oracle, cfg, precision=precision)
+    if precision == "f64":
+        _cmp_solve(g, o, 1e-11, 1e-9, True)
+        for which, j in ((0, 3), (1, 5), (0, 12), (1, 12)):
+            assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - o.get_slice(which, j))) < 1e-9, (which, j)
+        Hg, rg = g.scft_step(2.0, 2.0, 1); Ho, ro = o.scft_step(2.0, 2.0, 1)
+        assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9
+        g.cl_step(0.01, 1, 99, 0); o.cl_step(0.01, 1, 99, 0)
+        for x, y in zip(g.get_fields(), o.get_fields()):
+            assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    else:
+        g.propagate(); o.propagate()
+        Qg, pa, pb = g.density_operators(); Qo, oa, ob = o.density_operators()
+        assert abs(Qg - Qo) < 2e-4 * abs(Qo)
+        assert np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 and np.max(np.abs(pb.cpu().numpy() - ob)) < 2e-4

@@ -36,7 +36,12 @@ def test_argument_validation_without_gpu(libpath):
     both = B.make_params("diblock", fA=0.3, chiN=20.0, store_both=1)
     assert B.workspace_bytes((32, 32, 32), 100, both) > 2 * 101 * 32 ** 3 * 16        # store_both: every slice of q and q+
     assert B.workspace_bytes((32, 32, 32), 100, ok, "f32") < B.workspace_bytes((32, 32, 32), 100, ok)
+    # 1-D / 2-D grids are grids with dimensions of 1 (the ones do not change the memory layout)
+    assert B.workspace_bytes((64, 1, 1), 100, ok) == B.workspace_bytes((1, 1, 64), 100, ok) == B.workspace_bytes((1, 64, 1), 100, ok)
+    assert B.workspace_bytes((32, 16, 1), 100, ok) == B.workspace_bytes((1, 32, 16), 100, ok)
     for grid, Ns, p, status in [((32, 32, 12), 100, ok, 6),                           # not a power of two
+                                ((1, 1, 1), 100, ok, 6),
+                                ((4, 1, 1), 100, ok, 6),
                                 ((512, 8, 8), 100, ok, 6),
                                 ((32, 32, 32), 1, ok, 1),
                                 ((32, 32, 32), 10, B.make_params("diblock", fA=0.33, chiN=20.0), 1),    # fA*Ns not integer
