@@ -129,6 +129,9 @@ fts_status fts_set_option(fts_ctx* ctx, const char* key, long long value);
 /* Raw Philox4x32-10 block and the standard normal fts_cl_step draws for (seed, step, field, site), evaluated
  * ON THE DEVICE for n consecutive sites starting at site0; out_dev receives n doubles.  For tests. */
 fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out_dev, void* stream);
+/* The four raw 32-bit Philox4x32-10 words behind each of those normals (key = seed, counter = (site lo, site hi, step lo,
+ * field_id ^ (step hi << 8)); reading A-15): out_dev receives 4 n words.  For the bit-exact test. */
+fts_status fts_debug_philox(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, uint32_t* out_dev, void* stream);
 
 /* Measurement aids for bench.py.  fts_debug_fma_peak launches register-resident FMA chains (64 FMAs per thread per
  * iteration, 148*8 CTAs of 256 threads) and returns the number of FMAs issued, so the caller's own CUDA-event timing

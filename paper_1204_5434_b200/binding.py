@@ -16,7 +16,7 @@ STATUS = {0: "FTS_OK", 1: "FTS_EINVAL", 2: "FTS_ESTATE", 3: "FTS_EWORKSPACE", 4:
 MODELS = {"external": 0, "edwards": 1, "diblock": 2}
 EXPORTS = ["fts_workspace_bytes", "fts_create", "fts_destroy", "fts_set_fields", "fts_get_fields", "fts_propagate",
            "fts_propagate_steps", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
-           "fts_operators", "fts_set_option", "fts_debug_normals", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
+           "fts_operators", "fts_set_option", "fts_debug_normals", "fts_debug_philox", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
 
 
 class FtsParams(C.Structure):
@@ -56,6 +56,7 @@ def lib():
         L.fts_operators.argtypes = [vp, dp, dp, dp, vp]
         L.fts_set_option.argtypes = [vp, C.c_char_p, C.c_longlong]
         L.fts_debug_normals.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
+        L.fts_debug_philox.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
         L.fts_debug_fma_peak.argtypes = [C.c_int, C.c_int, vp, C.c_size_t, dp, vp]
         L.fts_launch_count.restype = C.c_uint64
         L.fts_last_error.argtypes = [vp]
@@ -182,6 +183,15 @@ def debug_normals(seed, step, field_id, site0, n, device="cuda:0"):
     if rc:
         raise FtsError("fts_debug_normals", rc)
     return out
+
+
+def debug_philox(seed, step, field_id, site0, n, device="cuda:0"):
+    """(n, 4) int64 tensor holding the raw 32-bit Philox words of sites site0 .. site0 + n - 1."""
+    out = torch.empty((n, 4), dtype=torch.int32, device=device)
+    rc = lib().fts_debug_philox(int(seed), int(step), int(field_id), int(site0), int(n), _p(out), _stream())
+    if rc:
+        raise FtsError("fts_debug_philox", rc)
+    return out.to(torch.int64) & 0xFFFFFFFF
 
 
 def launch_count():

@@ -927,4 +927,12 @@ fts_status fts_debug_normals(uint64_t seed, uint64_t step, uint32_t field_id, ui
     return cudaGetLastError() == cudaSuccess ? FTS_OK : FTS_ECUDA;
 }
 
+fts_status fts_debug_philox(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, uint32_t* out_dev, void* stream) {
+    if (!out_dev) return FTS_EINVAL;
+    if (n == 0) return FTS_OK;
+    philox_words_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, field_id, site0, n, out_dev);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? FTS_OK : FTS_ECUDA;
+}
+
 }  // extern "C"

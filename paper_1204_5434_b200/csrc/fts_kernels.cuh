@@ -270,6 +270,15 @@ __device__ __forceinline__ double normal_dev(uint64_t seed, uint64_t step, uint3
     const double u1 = (double)(m1 + 1) * 0x1p-53, u2 = (double)(m2 + 1) * 0x1p-53;
     return sqrt(-2.0 * log(u1)) * cos(2.0 * 3.14159265358979323846264338327950288 * u2);
 }
+// the four raw Philox words behind normal_dev, for the bit-exact comparison with the oracle (fts_debug_philox)
+__global__ void philox_words_kernel(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, uint32_t* out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint64_t site = site0 + i;
+    uint32_t o[4];
+    philox4x32_10((uint32_t)site, (uint32_t)(site >> 32), (uint32_t)step, field_id ^ ((uint32_t)(step >> 32) << 8), (uint32_t)seed, (uint32_t)(seed >> 32), o);
+    out[4 * i] = o[0]; out[4 * i + 1] = o[1]; out[4 * i + 2] = o[2]; out[4 * i + 3] = o[3];
+}
 __global__ void normals_kernel(uint64_t seed, uint64_t step, uint32_t field_id, uint64_t site0, size_t n, double* out) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[i] = normal_dev(seed, step, field_id, site0 + i);

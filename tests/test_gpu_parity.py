@@ -125,6 +125,26 @@ def test_philox_normals_match_oracle(B, oracle):
     assert np.max(np.abs(z - ref)) < 1e-13          # same Philox integers; libm vs CUDA log/cos differ by ulps
 
 
+def test_philox_words_bit_identical_over_a_million_counters(B, oracle):
+    """the device's and the oracle's Philox4x32-10 outputs are the same integers, for 2^20 counters: consecutive
+    sites across the 2^32 boundary of the site index, a step index with a high word, both field ids."""
+    import ctypes as C
+    n = 1 << 19
+    olib = oracle.lib()
+    c, k, o = (C.c_uint32 * 4)(), (C.c_uint32 * 2)(), (C.c_uint32 * 4)()
+    for seed, step, field, site0 in ((0x0123456789ABCDEF, 7, 0, 2 ** 32 - n // 2), (42, 2 ** 35 + 3, 1, 0)):
+        dev = B.debug_philox(seed, step, field, site0, n).cpu().numpy()
+        ref = np.empty((n, 4), np.int64)
+        k[0], k[1] = seed & 0xFFFFFFFF, seed >> 32
+        c[2], c[3] = step & 0xFFFFFFFF, field ^ (((step >> 32) << 8) & 0xFFFFFFFF)
+        for i in range(n):
+            site = site0 + i
+            c[0], c[1] = site & 0xFFFFFFFF, site >> 32
+            olib.oracle_philox4x32_10(c, k, o)
+            ref[i, 0], ref[i, 1], ref[i, 2], ref[i, 3] = o[0], o[1], o[2], o[3]
+        assert np.array_equal(dev, ref)
+
+
 @pytest.mark.parametrize("seidel", [0, 1])
 def test_scft_trajectory(B, oracle, seidel):
     cfg = inputs.config2(grid=(16, 16, 16), Ns=20)
@@ -294,24 +314,70 @@ def test_single_propagator_cubic_64(B, oracle, model):
     assert np.max(np.abs(g.get_slice(0, cfg.Ns).cpu().numpy() - o.get_slice(0, cfg.Ns))) < 1e-9
 
 
-@pytest.mark.parametrize("n,nsteps", [(128, 2), (256, 2)])
+CL_SEED = 20120454
+
+
+@pytest.fixture(scope="module")
+def oracle_cfg5s(oracle):
+    """Config 5s (128^3, Ns = 100, q and q+: 200 RQM4 steps) on the oracle, ONCE per session (~2 x 150 s on one core): a full
+    solve (Q, phi_A, phi_B) and the complex-Langevin step from the same fields (which solves again)."""
+    cfg = inputs.config5(128)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
+    o.set_fields(cfg.f0, cfg.f1)
+    o.propagate()
+    Q, pa, pb = o.density_operators()
+    qN = o.get_slice(0, cfg.Ns)
+    o.cl_step(cfg.dt, 0, CL_SEED, 0)
+    wp, wm = o.get_fields()
+    del o
+    return cfg, Q, pa, pb, qN, wp, wm
+
+
 @pytest.mark.parametrize("precision", ["f64", "f32"])
-def test_full_size_config5(B, oracle, n, nsteps, precision):
-    """BASELINE config 5 (256^3) and its 128^3 scaling point in the launch configuration bench.py times: oracle parity on
-    a truncated march (the oracle needs ~10 s per 256^3 step), then properties that hold at any size on the full march."""
-    cfg = inputs.config5(n)
+def test_config5s_full_oracle_solve_and_cl_step(B, oracle_cfg5s, precision):
+    """SURVEY 8(d), config 5s in the launch configuration bench.py times (TMA march, default store): Q to 1e-11 (2e-4 in
+    complex64), phi_A, phi_B and q(r,1) element-wise to 1e-9 (2e-4), and the fields after one fts_cl_step with identical Philox
+    noise to 1e-9 (2e-4), all against the oracle's full 200-step solve."""
+    cfg, Qo, oa, ob, qN, wpo, wmo = oracle_cfg5s
+    dt = torch.complex128 if precision == "f64" else torch.complex64
+    tq, tp = (1e-11, 1e-9) if precision == "f64" else (2e-4, 2e-4)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
+    g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
+    g.propagate()
+    Qg, pa, pb = g.density_operators()
+    assert abs(Qg - Qo) <= tq * abs(Qo), (Qg, Qo)
+    assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tp and np.max(np.abs(pb.cpu().numpy() - ob)) <= tp
+    assert np.max(np.abs(g.get_slice(0, cfg.Ns).cpu().numpy() - qN)) <= tp * max(1.0, np.max(np.abs(qN)))
+    g.cl_step(cfg.dt, 0, CL_SEED, 0)
+    wp, wm = g.get_fields()
+    assert np.max(np.abs(wp.cpu().numpy() - wpo)) <= tp * max(1.0, np.max(np.abs(wpo)))
+    assert np.max(np.abs(wm.cpu().numpy() - wmo)) <= tp * max(1.0, np.max(np.abs(wmo)))
+
+
+@pytest.fixture(scope="module")
+def oracle_cfg5_first8(oracle):
+    """Config 5 (256^3): the first 8 contour steps of q and q+ on the oracle (16 RQM4 steps of 2^24 points, ~100 s), once."""
+    cfg = inputs.config5(256)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
+    o.set_fields(cfg.f0, cfg.f1)
+    o.propagate(8)
+    sl = {(w, j): o.get_slice(w, j) for w in (0, 1) for j in (1, 8)}
+    del o
+    return cfg, sl
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_config5_truncated_march_and_invariants(B, oracle_cfg5_first8, precision):
+    """Config 5 (256^3) in the launch configuration bench.py times: slices 1 and 8 of both propagators against the oracle
+    (first 8 steps), then properties that hold at any size on the full march with every slice kept."""
+    cfg, sl = oracle_cfg5_first8
     dt = torch.complex128 if precision == "f64" else torch.complex64
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=1, **_kw(cfg))
     g.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
-    g.propagate(nsteps)
-    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
-    o.set_fields(cfg.f0, cfg.f1)
-    o.propagate(nsteps)
+    g.propagate(8)
     tol = 1e-10 if precision == "f64" else 2e-4
-    for which in (0, 1):
-        ref = o.get_slice(which, nsteps)
-        assert np.max(np.abs(g.get_slice(which, nsteps).cpu().numpy() - ref)) <= tol * max(1.0, np.max(np.abs(ref))), which
-    del o
+    for (which, j), ref in sl.items():
+        assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - ref)) <= tol * max(1.0, np.max(np.abs(ref))), (which, j)
     g.propagate()
     Q, pa, pb = g.density_operators()
     rel = 1e-11 if precision == "f64" else 2e-4
@@ -320,6 +386,13 @@ def test_full_size_config5(B, oracle, n, nsteps, precision):
         assert abs(Qj - Q) <= rel * abs(Q), j
     assert abs(complex(pa.to(torch.complex128).mean().item()) - cfg.fA) <= rel
     assert abs(complex((pa + pb).to(torch.complex128).mean().item()) - 1.0) <= rel
+    # the default (meet-in-the-middle) store gives the same Q and densities bit for bit: the arithmetic does not depend on it
+    del g
+    g2 = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
+    g2.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
+    g2.propagate()
+    Q2, pa2, pb2 = g2.density_operators()
+    assert Q2 == Q and torch.equal(pa2, pa) and torch.equal(pb2, pb)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -376,6 +449,7 @@ def test_config2_scft_full_size(B, oracle):
     assert res[-1] < res[0]                            # the relaxation makes progress
     _invariants(g, cfg, 1e-11)
     _developed_solve_parity(B, oracle, cfg)
+    _developed_solve_parity(B, oracle, cfg, precision="f32", tolQ=2e-4, tolphi=2e-4)      # complex64 at full size
 
 
 @pytest.mark.parametrize("precision", ["f64", "f32"])
@@ -383,7 +457,14 @@ def test_config3_scft_full_size(B, oracle, precision):
     """64^3, Ns = 200 (jA = 70), q+ batched with q: 30 Seidel iterations on the GPU (invariants), one solve at developed
     fields against the oracle."""
     cfg = inputs.config3()
-    g, _ = _pair(B, oracle, cfg, precision=precision)
+    g, o = _pair(B, oracle, cfg, precision=precision)
+    if precision == "f64":                             # one Seidel iteration side by side (2 x 400 RQM4 steps on the oracle, ~75 s)
+        Hg, rg = g.scft_step(*cfg.dt_scft, 1)
+        Ho, ro = o.scft_step(*cfg.dt_scft, 1)
+        assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9
+        for x, y in zip(g.get_fields(), o.get_fields()):
+            assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    del o
     for it in range(30):
         H, r = g.scft_step(*cfg.dt_scft, 1)
     assert np.isfinite(H.real) and max(r) < 1.0
@@ -407,6 +488,7 @@ def test_config4_edwards_cl_full_size(B, oracle):
         g.cl_step(cfg.dt, 0, 4242, step)
     _invariants(g, cfg, 1e-11)
     _developed_solve_parity(B, oracle, cfg, operators=True)
+    _developed_solve_parity(B, oracle, cfg, precision="f32", tolQ=2e-4, tolphi=2e-4)      # complex64 at full size
 
 
 @pytest.mark.parametrize("model", ["diblock", "edwards"])
@@ -534,3 +616,19 @@ def test_one_and_two_dimensional_grids(B, oracle, grid, cell, precision):
         Qg, pa, pb = g.density_operators(); Qo, oa, ob = o.density_operators()
         assert abs(Qg - Qo) < 2e-4 * abs(Qo)
         assert np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 and np.max(np.abs(pb.cpu().numpy() - ob)) < 2e-4
+
+
+@pytest.mark.parametrize("grid", [(256, 8, 8), (8, 128, 16), (16, 8, 256), (128, 16, 8)])
+def test_filter_passes_at_long_pencils(B, oracle, grid):
+    """pass_kernel (the 3-D filters of the SCFT / Eq. 11 updates and the Laplacian of Pi) at pencil lengths 128 and 256 along
+    each dimension: one SCFT iteration, one semi-implicit CL step and the operators H, mu, Pi against the oracle."""
+    cfg = inputs.small_diblock(grid=grid, cell=(7.0, 5.0, 6.0), Ns=8, fA=0.5)
+    g, o = _pair(B, oracle, cfg)
+    Hg, rg = g.scft_step(2.0, 2.0, 0); Ho, ro = o.scft_step(2.0, 2.0, 0)
+    assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9
+    g.cl_step(0.01, 1, 5, 3); o.cl_step(0.01, 1, 5, 3)
+    for x, y in zip(g.get_fields(), o.get_fields()):
+        assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    g.propagate(); o.propagate()
+    for x, y in zip(g.operators(), o.operators()):
+        assert abs(x - y) < 1e-9 * max(1.0, abs(y))
