@@ -48,6 +48,7 @@ def make_workload(name):
 
 
 def rqm4_steps_per_step(cfg, kind):
+    """RQM4 steps of the METHOD per bench step (q and q+ counted separately, also when the real-field path marches them packed)."""
     nprop = 2 if cfg.model == "diblock" else 1
     solves = 2 if kind == "scft" else 1          # seidel = 1: two propagator solves per SCFT iteration
     return nprop * cfg.Ns * solves
@@ -229,6 +230,8 @@ def run_gpu(args):
     M, nprop = int(np.prod(cfg.grid)), (2 if cfg.model == "diblock" else 1)
     E = 16 if prec == "f64" else 8
     opts = dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt)
+    if kind == "scft" and "real_fields" not in opts:
+        opts["real_fields"] = 1                     # SCFT fields are real: q and q+ share one packed march (N1)
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, options=opts, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
     host = [torch.from_numpy(np.ascontiguousarray(f)).to(cdt).pin_memory() for f in (cfg.f0, cfg.f1) if f is not None]
     devf = [h.to(dev) for h in host]
@@ -340,7 +343,7 @@ def run_gpu(args):
                               "frac_of_floor": t_hbm / t_step}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-           "config": config_dict(cfg, kind, prec, world),
+           "config": config_dict(cfg, kind, prec, world, {"options": opts} if opts else None),
            "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
                                                                                       "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),

@@ -37,7 +37,8 @@ struct Ctx {
     size_t counters_bytes;
     int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
     // options (fts_set_option; no environment variables are read)
-    struct { int march; long long slab_bytes; int lag, interleave, tz, skew; } opt;
+    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields; } opt;
+    int packed;                   // N1 real-field fast path active: one march of z = q + i q+ (fts_march.cuh); nprop is then 1
     // TMA march for large cubic grids (fts_march2.cuh)
     int v2, v2_lag, v2_skew, v2_occ;
     March2Maps maps;
@@ -294,6 +295,10 @@ static std::vector<Phase> make_template(int nprop, int nchunks, int lag, bool in
     return v;
 }
 
+// Boltzmann-factor fields: per species, or (packed mode) per species pair; the pair fields 2, 3 live in the second propagator's
+// F and H, which the packed march does not use
+static const void* e4_field(const Ctx* c, int i) { return i < 2 ? c->e4[i] : (c->packed ? (i == 2 ? c->F[1] : c->H[1]) : c->e4[i - 2]); }
+
 static DensArgs dens_args(const Ctx* c, int nsteps) {
     DensArgs D;
     for (int b = 0; b < 2; ++b) for (int a = 0; a < 2; ++a) D.acc[b][a] = c->acc[b][a];
@@ -304,7 +309,9 @@ static DensArgs dens_args(const Ctx* c, int nsteps) {
 template <class T>
 static void fill_march_args(const Ctx* c, MarchArgs& A, int nsteps) {
     std::memset(&A, 0, sizeof A);
-    for (int b = 0; b < 2; ++b) { A.q[b] = c->q[b]; A.F[b] = c->F[b]; A.H[b] = c->H[b]; A.e4[b] = c->e4[b]; }
+    for (int b = 0; b < 2; ++b) { A.q[b] = c->q[b]; A.F[b] = c->F[b]; A.H[b] = c->H[b]; }
+    for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
+    A.nprop = c->nprop; A.packed = c->packed;
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; A.tw[d] = c->dim[d].tw; A.g[d] = c->g[d]; }
     A.M = (long long)c->M; A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nsteps = nsteps;
     A.done = c->counters; A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
@@ -413,7 +420,8 @@ static fts_status plan_march2(Ctx* c) {
     for (int b = 0; b < 2 && ok; ++b) {
         const int pb = b < c->nprop ? b : 0;
         ok = ok && make_tile_map(c, &c->maps.x[M2_MAP_F + b], c->F[pb], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_H + b], c->H[pb], 1, true) &&
-             make_tile_map(c, &c->maps.x[M2_MAP_E + b], c->e4[b], 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_Q + b], c->q[pb], c->nslots, true) &&
+             make_tile_map(c, &c->maps.x[M2_MAP_E + b], (void*)e4_field(c, b), 1, true) && make_tile_map(c, &c->maps.x[M2_MAP_E + 2 + b], (void*)e4_field(c, 2 + b), 1, true) &&
+             make_tile_map(c, &c->maps.x[M2_MAP_Q + b], c->q[pb], c->nslots, true) &&
              make_tile_map(c, &c->maps.y[0 + b], c->F[pb], 1, false) && make_tile_map(c, &c->maps.y[2 + b], c->H[pb], 1, false);
     }
     if (!ok) {
@@ -441,7 +449,9 @@ static fts_status plan_march2(Ctx* c) {
 template <class T>
 static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     March2Args A; std::memset(&A, 0, sizeof A);
-    for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; A.e4[b] = c->e4[b]; }
+    for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; }
+    for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
+    A.packed = c->packed;
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; }
     A.tw = c->dim[0].tw2;
     A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nprop = c->nprop; A.nsteps = nsteps; A.lag = c->v2_lag; A.skew = c->v2_skew;
@@ -507,15 +517,21 @@ template <class T>
 static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
     const size_t M = c->M; const int Ns = c->Ns;
     const double ds = 1.0 / Ns;
-    boltzmann_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)c->e4[0], (cplx<T>*)c->e4[1], (int)M, c->P.model, ds / 4);
+    int* flag = (int*)((char*)c->counters + c->counters_bytes - 128);
+    if (c->packed)
+        boltzmann_packed_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)e4_field(c, 0), (cplx<T>*)e4_field(c, 1),
+                                                                (cplx<T>*)e4_field(c, 2), (cplx<T>*)e4_field(c, 3), (int)M, ds / 4, flag);
+    else
+        boltzmann_kernel<T><<<ew_blocks(M), 256, 0, st>>>((const cplx<T>*)c->f0, (const cplx<T>*)c->f1, (cplx<T>*)c->e4[0], (cplx<T>*)c->e4[1], (int)M, c->P.model, ds / 4);
     g_launches += 1;
     CK(cudaGetLastError());
     fts_status rc = march_t<T>(c, nsteps, st); if (rc) return rc;
     // S7 (Eq. 4): Q = (1/M) sum_x q_Ns(x), fixed-order tree
     // (a march that gave up on a dependency leaves its error flag set: Q then becomes NaN, so that everything downstream of it --
     // densities, field updates, operators -- is visibly invalid, and every call that returns scalars reports FTS_ECUDA)
-    CK((reduce<T, RED_SUM>(c, (const cplx<T>*)c->q[0] + (size_t)slice_slot(nsteps, c->keep) * M, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st,
-                           (const int*)((const char*)c->counters + c->counters_bytes - 128))));
+    const cplx<T>* qlast = (const cplx<T>*)c->q[0] + (size_t)slice_slot(nsteps, c->keep) * M;
+    if (c->packed) CK((reduce<T, RED_SUMRE>(c, qlast, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st, flag)));      // z = q + i q+: Q = mean Re z
+    else CK((reduce<T, RED_SUM>(c, qlast, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st, flag)));
     c->marched = nsteps; c->have_prop = true; c->have_phi = false;
     return FTS_OK;
 }
@@ -524,6 +540,12 @@ static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
 // the march's T items.  Written to phiA / phiB (the context's own phi fields or the caller's).
 template <class T>
 static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
+    if (c->packed) {
+        density_finish_packed_kernel<T><<<ew_blocks(c->M), 256, 0, st>>>((const cplx<T>*)c->acc[0][0], (int)c->M, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA, (cplx<T>*)phiB);
+        g_launches += 1;
+        CK(cudaGetLastError());
+        return FTS_OK;
+    }
     const bool two = c->nprop == 2;
     density_finish_kernel<T><<<ew_blocks(c->M), 256, 0, st>>>((const cplx<T>*)c->acc[0][0], two ? (const cplx<T>*)c->acc[1][0] : nullptr,
                                                              two ? (const cplx<T>*)c->acc[0][1] : nullptr, two ? (const cplx<T>*)c->acc[1][1] : nullptr,
@@ -553,6 +575,7 @@ static fts_status read_scalars(Ctx* c, double* host, int n, cudaStream_t st) {
     CK(cudaMemcpyAsync(host, c->scal, n * sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(&flag, (char*)c->counters + c->counters_bytes - 128, sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    if (flag == 3) { c->err = "real_fields is set but the fields have imaginary parts"; return FTS_EINVAL; }
     if (flag) { c->err = "march kernel: a dependency wait timed out (results invalid)"; return FTS_ECUDA; }
     return FTS_OK;
 }
@@ -571,6 +594,7 @@ static fts_status scft_step_t(Ctx* c, double dtp, double dtm, int seidel, double
     rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
     add_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, (const cplx<T>*)c->G[0], M);
     g_launches += 1;
+    if (c->packed) { real_part_kernel<T><<<nb, 256, 0, st>>>((cplx<T>*)c->f0, M); g_launches += 1; }      // the complex filter leaves rounding noise in Im
     if (seidel) {
         rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
         rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
@@ -633,6 +657,7 @@ static fts_status operators_t(Ctx* c, double* Ho, double* muo, double* Pio, cuda
     const cplx<T>* q = (const cplx<T>*)c->q[0];
     const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];
     fts_status rc;
+    if (Pio && c->packed) { c->err = "Pi is not available with real_fields"; return FTS_EUNSUPPORTED; }
     if (Pio && c->keep != Ns) { c->err = "Pi needs every slice of q and q+: create the context with store_both = 1"; return FTS_ESTATE; }
     if (Pio) {                                             // K_j = (1/M) sum_x q+_{Ns-j} Laplacian(q_j)
         Filt f; f.type = FILT_NEGK2; f.a = 1.0; f.b = f.c = 0.0;
@@ -805,7 +830,8 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->keep = Lo.keep; c->nslots = Lo.nslots;
     c->have_fields = c->have_prop = c->have_phi = false; c->marched = 0; c->occ = 0;
-    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1;
+    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0;
+    c->packed = 0;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
     if (!rc) rc = replan(c);
@@ -826,6 +852,13 @@ fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     else if (!std::strcmp(key, "skew")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.skew = (int)value; }
     else if (!std::strcmp(key, "interleave")) c->opt.interleave = value != 0;
     else if (!std::strcmp(key, "tz")) { if (value != 0 && value != 8 && value != 16) return FTS_EINVAL; c->opt.tz = (int)value; }
+    else if (!std::strcmp(key, "real_fields")) {
+        if (value != 0 && value != 1) return FTS_EINVAL;
+        if (value && c->P.model != FTS_MODEL_DIBLOCK) return FTS_EUNSUPPORTED;      // one propagator: nothing to pack
+        c->opt.real_fields = (int)value;
+        c->packed = (int)value;
+        c->nprop = c->packed ? 1 : c->nspecies;
+    }
     else return FTS_EINVAL;
     if (c->opt.march == FTS_MARCH_TMA && !v2_shape_ok(c)) { c->opt = old; return FTS_EUNSUPPORTED; }
     c->occ = 0;
@@ -878,6 +911,14 @@ fts_status fts_get_slice(fts_ctx* c, int which, int j, void* out, void* stream) 
     if (!c || !out || which < 0 || which > 1 || j < 0 || j > c->Ns) return FTS_EINVAL;
     if (!c->have_prop || j > c->marched) return FTS_ESTATE;
     if (j > c->keep && j != c->marched) { c->err = "slice not retained by the meet-in-the-middle store (store_both = 0)"; return FTS_ESTATE; }
+    if (c->packed) {
+        const char* z = (const char*)c->q[0] + (size_t)slice_slot(j, c->keep) * c->M * c->esz;
+        if (c->prec == FTS_F64) unpack_kernel<double><<<ew_blocks(c->M), 256, 0, (cudaStream_t)stream>>>((const cplx<double>*)z, (cplx<double>*)out, (int)c->M, which);
+        else unpack_kernel<float><<<ew_blocks(c->M), 256, 0, (cudaStream_t)stream>>>((const cplx<float>*)z, (cplx<float>*)out, (int)c->M, which);
+        g_launches += 1;
+        CK(cudaGetLastError());
+        return FTS_OK;
+    }
     const char* base = (const char*)c->q[which == 1 ? c->nprop - 1 : 0];
     CK(cudaMemcpyAsync(out, base + (size_t)slice_slot(j, c->keep) * c->M * c->esz, c->M * c->esz, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return FTS_OK;
@@ -895,6 +936,7 @@ fts_status fts_cl_step(fts_ctx* c, double dt, int scheme, uint64_t seed, uint64_
     if (!c || !(dt > 0) || scheme < 0 || scheme > 1) return FTS_EINVAL;
     if (c->P.model == FTS_MODEL_EXTERNAL) return FTS_EUNSUPPORTED;
     if (!c->have_fields) return FTS_ESTATE;
+    if (c->packed) { c->err = "complex Langevin fields are complex: clear the real_fields option first"; return FTS_ESTATE; }
     cudaStream_t st = (cudaStream_t)stream;
     return DISPATCH(cl_step_t<double>(c, dt, scheme, seed, step, st), cl_step_t<float>(c, dt, scheme, seed, step, st));
 }

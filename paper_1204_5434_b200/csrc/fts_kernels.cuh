@@ -178,16 +178,50 @@ __global__ void boltzmann_kernel(const cplx<T>* f0, const cplx<T>* f1, cplx<T>* 
     }
 }
 
+// N1 real-field fast path (fts_march.cuh, cmul): packed factor fields (exp(-w_a ds/4), exp(-w_b ds/4)) for the species pairs
+// (a, b) = (A,A), (A,B), (B,A), (B,B) -> out[2a + b]; w_A = W+ - W-, w_B = W+ + W- from the REAL parts of the stored fields.
+// A field that is not real (|Im| > 1e-12 (1 + |Re|)) raises *flag to 3: the declaration "real_fields" was wrong.
+template <class T>
+__global__ void boltzmann_packed_kernel(const cplx<T>* f0, const cplx<T>* f1, cplx<T>* o0, cplx<T>* o1, cplx<T>* o2, cplx<T>* o3, int M, double ds4, int* flag) {
+    bool bad = false;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        const double p = (double)f0[i].x, m = (double)f1[i].x;
+        bad = bad || fabs((double)f0[i].y) > 1e-12 * (1.0 + fabs(p)) || fabs((double)f1[i].y) > 1e-12 * (1.0 + fabs(m));
+        const T ea = (T)exp(-(p - m) * ds4), eb = (T)exp(-(p + m) * ds4);
+        o0[i] = mk<T>(ea, ea); o1[i] = mk<T>(ea, eb); o2[i] = mk<T>(eb, ea); o3[i] = mk<T>(eb, eb);
+    }
+    if (bad) atomicExch(flag, 3);
+}
+// slice of q (which = 0) or q+ (which = 1) out of the packed slice z = q + i q+
+template <class T>
+__global__ void unpack_kernel(const cplx<T>* z, cplx<T>* out, int M, int which) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) out[i] = mk<T>(which ? z[i].y : z[i].x, (T)0);
+}
+// packed sums (A, B) as (re, im) -> phi_A, phi_B = (ds / Q) sums, Q real
+template <class T>
+__global__ void density_finish_packed_kernel(const cplx<T>* acc, int M, const double* Qdev, double ds, cplx<T>* phiA, cplx<T>* phiB) {
+    const double f = ds / Qdev[0];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) {
+        phiA[i] = mk<T>((T)((double)acc[i].x * f), (T)0);
+        phiB[i] = mk<T>((T)((double)acc[i].y * f), (T)0);
+    }
+}
+template <class T>
+__global__ void real_part_kernel(cplx<T>* w, int M) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < M; i += gridDim.x * blockDim.x) w[i].y = (T)0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // deterministic reductions: fixed grid, fixed per-thread order, fixed shared-memory tree
 // ------------------------------------------------------------------------------------------------
-enum { RED_SUM = 0, RED_SUMSQ = 1, RED_PROD = 2, RED_DIBLOCK_H = 3, RED_MAXABS = 4 };
+enum { RED_SUM = 0, RED_SUMSQ = 1, RED_PROD = 2, RED_DIBLOCK_H = 3, RED_MAXABS = 4, RED_SUMRE = 5 };
 constexpr int RED_BLOCKS = 592, RED_THREADS = 256;     // 4 CTAs per SM on 148 SMs
 
 template <class T, int OP>
 __device__ __forceinline__ double2 red_value(const cplx<T>* a, const cplx<T>* b, int i, double p) {
     const double ax = (double)a[i].x, ay = (double)a[i].y;
     if constexpr (OP == RED_SUM) return make_double2(ax, ay);
+    else if constexpr (OP == RED_SUMRE) return make_double2(ax, 0.0);
     else if constexpr (OP == RED_SUMSQ) return make_double2(ax * ax - ay * ay, 2.0 * ax * ay);
     else if constexpr (OP == RED_PROD) { const double bx = (double)b[i].x, by = (double)b[i].y; return make_double2(ax * bx - ay * by, ax * by + ay * bx); }
     else if constexpr (OP == RED_DIBLOCK_H) {           // W-^2/chiN - W+ with a = W+, b = W-, p = 1/chiN   (Eq. 3)

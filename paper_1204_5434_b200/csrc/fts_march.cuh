@@ -58,13 +58,31 @@ struct DensArgs {
 };
 __host__ __device__ inline int slice_slot(int s, int keep) { return s <= keep ? s : keep + 1; }
 
+// N1, real-field fast path (the SCFT fields are real).  With real w_A, w_B the propagators
+// q and q+ are real, and because every diffusion factor F^-1 exp(-k^2 ds) F is a REAL linear operator, the two marches can
+// share one complex march of z = q + i q+:  the Boltzmann multiplies act component-wise, (Re z e_q, Im z e_q+), with the
+// factor field packed as (exp(-w_{alpha(s)} ds/4), exp(-w_{alpha+(s)} ds/4)) for the species pair of step s.  Half the
+// transforms, half the slices.  species_index() names the factor field of a step; cmul() is the multiply of either mode.
+__host__ __device__ inline int species_index(int packed, int nspecies, int jA, int Ns, int b, int step) {
+    if (nspecies != 2) return 0;
+    const int sq = step >= jA ? 1 : 0, sqd = step < Ns - jA ? 1 : 0;       // O5 / O6 block schedule of q and of q+
+    if (packed) return 2 * sq + sqd;
+    return b == 0 ? sq : sqd;
+}
+template <class T> __device__ __forceinline__ cplx<T> cmul(cplx<T> a, cplx<T> e, bool componentwise) {
+    return componentwise ? mk<T>(a.x * e.x, a.y * e.y) : a * e;
+}
+
 struct MarchArgs {
-    void* q[2]; void* F[2]; void* H[2]; const void* e4[2];
+    void* q[2]; void* F[2]; void* H[2];
+    const void* e4[4];          // Boltzmann factors exp(-w ds/4) per species; packed mode: per (species of q, species of q+) pair
     const void* tab[3][2];      // per dimension: exp(-k_d^2 ds)/N_d, exp(-k_d^2 ds/2)/N_d
     const void* tw[3];          // per dimension: inter-stage twiddles, per-(register, thread) layout
     int g[3];
     long long M;
     int Ns, jA, nspecies, nsteps;
+    int nprop;                  // propagators marched (2 = diblock q and q+; 1 otherwise, and in packed mode)
+    int packed;                 // N1 real-field fast path: ONE complex march of z = q + i q+ (see cmul_mode)
     int nchunks, planes;        // x-slabs and planes per slab
     const Phase* phases; int nphases; int tickets_per_round; int round0, round1;   // rounds [round0, round1]
     int ntT, nY1, nZ, nY2;      // tickets of one T phase / of one slab's Y1, Z, Y2 phase
@@ -241,7 +259,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         auto dependency2 = [&](const Phase& ph, int s, unsigned& need) -> const unsigned* {
             need = 0;
             if (ph.kind != PH_T || !A.dens.on) return nullptr;
-            const int b = ph.prop_off & 1, nprop = A.nspecies == 2 ? 2 : 1;      // diblock: two propagators
+            const int b = ph.prop_off & 1, nprop = A.nprop;
             if (nprop == 2 ? (b == 0 ? s <= A.dens.half : s < A.dens.half) : s <= A.dens.half) return nullptr;
             need = (unsigned)A.ntT;
             return A.done + ((size_t)(nprop == 2 ? 1 - b : 0) * (A.Ns + 1) + (A.Ns - s)) * C2;
@@ -372,10 +390,8 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         cp_async_commit();
     };
     // species of contour step `step` of propagator b (O5 / O6 block schedule)
-    auto species = [&](int b, int step) -> int {
-        if (A.nspecies != 2) return 0;
-        return b == 0 ? (step >= A.jA ? 1 : 0) : (step < A.Ns - A.jA ? 1 : 0);
-    };
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.jA, A.Ns, b, step); };
+    const bool cw = A.packed != 0;
 
     int cur_dim = -1;
     bool cur_pref = false;
@@ -437,13 +453,18 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
             const bool keep = c.s <= A.dens.keep || c.s == A.nsteps;
             C* qs = static_cast<C*>(A.q[c.b]) + (long long)slice_slot(c.s, A.dens.keep) * A.M;
             // density pair of this slice (DensArgs): partner slice and Simpson weights
-            const bool two = A.nspecies == 2;
+            const bool two = A.nprop == 2;
             const int h = A.dens.half, jp = (two && c.b == 1) ? A.Ns - c.s : c.s;      // contour index j of the pair (j, Ns - j)
             const bool dens = A.dens.on && (two ? (c.b == 0 ? c.s > h : c.s >= h) : c.s >= h);
             const bool self = !two && c.s == h;
             const C* partner = static_cast<const C*>(A.q[two ? 1 - c.b : 0]) + (long long)(A.Ns - c.s) * A.M;      // stored: Ns - s <= keep
             double wA = 0.0, wB = 0.0;
-            if (dens) { wA = A.dens.cA[jp]; wB = A.dens.cB[jp]; if (!two && !self) wA += A.dens.cA[A.Ns - jp]; }
+            double wA2 = 0.0, wB2 = 0.0;                              // packed mode: the mirror pair (Ns - s, s)
+            if (dens) {
+                wA = A.dens.cA[jp]; wB = A.dens.cB[jp];
+                if (cw) { if (!self) { wA2 = A.dens.cA[A.Ns - jp]; wB2 = A.dens.cB[A.Ns - jp]; } }
+                else if (!two && !self) wA += A.dens.cA[A.Ns - jp];
+            }
             C* accA = static_cast<C*>(A.dens.acc[c.b][0]); C* accB = static_cast<C*>(A.dens.acc[c.b][1]);
             const C* e4s = static_cast<const C*>(A.e4[sp_now]);
             const bool reload = !combine || sp_now != sp_prev;
@@ -454,20 +475,27 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
                 if (combine) {                                        // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
                     e = s_stash[r * NT + tid];
                     const C f = s_pre[r * NT + tid];
-                    const C h = v[r] * e;
+                    const C h = cmul(v[r], e, cw);
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                 }
                 if (c.active && keep) stcg(qs + i, v[r]);             // the slice store IS the step's output write
                 if (dens && c.active) {                               // Eq. 8: this slice times the stored partner, weighted, into the sums
-                    const C pr = v[r] * (self ? v[r] : ldcg(partner + i));
-                    if (wA != 0.0) { const C a = ldcg(accA + i); stcg(accA + i, mk<T>(a.x + (T)wA * pr.x, a.y + (T)wA * pr.y)); }
-                    if (wB != 0.0) { const C a = ldcg(accB + i); stcg(accB + i, mk<T>(a.x + (T)wB * pr.x, a.y + (T)wB * pr.y)); }
+                    const C zp = self ? v[r] : ldcg(partner + i);
+                    if (cw) {                                         // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
+                        const T p1 = v[r].x * zp.y, p2 = zp.x * v[r].y;
+                        const C a = ldcg(accA + i);
+                        stcg(accA + i, mk<T>(a.x + (T)wA * p1 + (T)wA2 * p2, a.y + (T)wB * p1 + (T)wB2 * p2));
+                    } else {
+                        const C pr = v[r] * zp;
+                        if (wA != 0.0) { const C a = ldcg(accA + i); stcg(accA + i, mk<T>(a.x + (T)wA * pr.x, a.y + (T)wA * pr.y)); }
+                        if (wB != 0.0) { const C a = ldcg(accB + i); stcg(accB + i, mk<T>(a.x + (T)wB * pr.x, a.y + (T)wB * pr.y)); }
+                    }
                 }
                 if (start) {
                     if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
-                    const C hb = v[r] * e;
+                    const C hb = cmul(v[r], e, cw);
                     s_stash[r * NT + tid] = hb;
-                    v[r] = hb * e;
+                    v[r] = cmul(hb, e, cw);
                 }
             }
             return start;
@@ -484,7 +512,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         bool run = true;
         if (kind == PH_T && ((const volatile int*)s_item[slot])[0] == 0) {      // q(x,0) = 1, q+(x,s=1) = 1
 #pragma unroll
-            for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, 0);
+            for (int r = 0; r < EPT; ++r) v[r] = mk<T>(1, cw ? 1 : 0);      // packed: z_0 = q_0 + i q+_0 = 1 + i
             run = emit_q_and_start(false);
             stage_next();
             st = 1;
@@ -516,7 +544,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
 #pragma unroll
                 for (int r = 0; r < EPT; ++r) {
                     const C e = s_stash[r * NT + tid];
-                    v[r] = v[r] * (e * e);
+                    v[r] = cmul(v[r], cmul(e, e, cw), cw);
                 }
                 if (job == 0) { store_tile(0); run = false; }
                 st = 1;

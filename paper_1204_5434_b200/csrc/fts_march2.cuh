@@ -36,18 +36,19 @@ namespace fts {
 
 enum { M2_NBUF = 3, M2_RING = 4, M2_NT = 128, M2_LAUNCH = 192 };
 enum { M2_FIRST = 1, M2_FIN = 2, M2_START = 4, M2_RELOAD = 8, M2_JOBH = 16, M2_KEEP = 32, M2_DENS = 64 };
-enum { M2_MAP_F = 0, M2_MAP_H = 2, M2_MAP_E = 4, M2_MAP_Q = 6 };     // + propagator (F, H, Q) or species (E)
+enum { M2_MAP_F = 0, M2_MAP_H = 2, M2_MAP_E = 4, M2_MAP_Q = 8 };     // + propagator (F, H, Q) or factor-field index (E, 0..3)
 
 struct March2Maps {
-    CUtensorMap x[8];            // x tiles: box {16 scalars, 1, N, 1} of F0 F1 H0 H1 E0 E1 Q0 Q1
+    CUtensorMap x[10];           // x tiles: box {16 scalars, 1, N, 1} of F0 F1 H0 H1 E0 E1 E2 E3 Q0 Q1
     CUtensorMap y[4];            // y tiles: box {16 scalars, N, 1, 1} of F0 F1 H0 H1
 };
 
 struct March2Args {
-    void* F[2]; void* H[2]; const void* e4[2];
+    void* F[2]; void* H[2]; const void* e4[4];
     const void* tab[3][2];       // per dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
     const void* tw;              // twiddles of the twisted second stage, tw2[slot * R1 + k1] (fts_pencil.h)
     int Ns, jA, nspecies, nprop, nsteps, lag, skew;
+    int packed;                  // N1 real-field fast path: one march of z = q + i q+ (fts_march.cuh, cmul)
     const void* q[2];            // slice stores (the density partner is read straight from global memory)
     DensArgs dens;               // S6: Simpson density sums accumulated by the T items (fts_march.cuh)
     unsigned* ticket;
@@ -287,10 +288,8 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
     __syncthreads();
 
     const M2Sched<T, N> sched(A.nprop, A.lag, A.skew, A.nsteps);
-    auto species = [&](int b, int step) -> int {                    // O5 / O6 block schedule
-        if (A.nspecies != 2) return 0;
-        return b == 0 ? (step >= A.jA ? 1 : 0) : (step < A.Ns - A.jA ? 1 : 0);
-    };
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.jA, A.Ns, b, step); };      // O5 / O6 block schedule
+    const bool cw = A.packed != 0;
     auto nbuf_of = [](int kind) { return kind == PH_T ? 3 : (kind == PH_Z ? 2 : 1); };
     // TMA coordinates of sub-tile g of a strided item (c0 in scalars), and the byte offset of a z item inside a field
     auto xcoord = [](int idx, int g, int& c0, int& c1) { const int tile = idx * Cfg::G + g; c0 = (tile % (N / 8)) * 16; c1 = tile / (N / 8); };
@@ -510,13 +509,14 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
             }
             if (reload) e4s = static_cast<const C*>(A.e4[dv->spS]);     // block junction: the new species' factors straight from global memory
             // S6 (Eq. 8, DensArgs): this slice times the stored partner slice, Simpson-weighted, into the sums
-            const C* partner = nullptr; C* accA = nullptr; C* accB = nullptr; T wA = 0, wB = 0; bool self = false;
+            const C* partner = nullptr; C* accA = nullptr; C* accB = nullptr; T wA = 0, wB = 0, wA2 = 0, wB2 = 0; bool self = false;
             if (dens) {
                 const int b = dv->b, s = dv->s; const bool two = A.nprop == 2;
                 const int jp = (two && b == 1) ? A.Ns - s : s;
                 self = !two && s == A.dens.half;
                 double a = A.dens.cA[jp]; const double bb = A.dens.cB[jp];
-                if (!two && !self) a += A.dens.cA[A.Ns - jp];
+                if (cw) { if (!self) { wA2 = (T)A.dens.cA[A.Ns - jp]; wB2 = (T)A.dens.cB[A.Ns - jp]; } }
+                else if (!two && !self) a += A.dens.cA[A.Ns - jp];
                 wA = (T)a; wB = (T)bb;
                 partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N;
                 accA = static_cast<C*>(A.dens.acc[b][0]); accB = static_cast<C*>(A.dens.acc[b][1]);
@@ -526,21 +526,28 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                 C e = L.ld(pe + r * TPP * RB);
                 if (fin) {
                     const C f = L.ld(pf + r * TPP * RB);
-                    const C h = v[r] * e;
+                    const C h = cmul(v[r], e, cw);
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
-                } else v[r] = mk<T>(1, 0);                              // q(x,0) = 1, q+(x,s=1) = 1
+                } else v[r] = mk<T>(1, cw ? 1 : 0);                              // q(x,0) = 1, q+(x,s=1) = 1
                 L.st(pq + r * TPP * RB, v[r]);
                 if (dens) {
                     const int gi = gbase + r * TPP * N * N;
-                    const C pr = v[r] * (self ? v[r] : ldcg(partner + gi));
-                    if (wA != (T)0) { const C a = ldcg(accA + gi); stcg(accA + gi, mk<T>(a.x + wA * pr.x, a.y + wA * pr.y)); }
-                    if (wB != (T)0) { const C a = ldcg(accB + gi); stcg(accB + gi, mk<T>(a.x + wB * pr.x, a.y + wB * pr.y)); }
+                    const C zp = self ? v[r] : ldcg(partner + gi);
+                    if (cw) {                                           // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
+                        const T p1 = v[r].x * zp.y, p2 = zp.x * v[r].y;
+                        const C a = ldcg(accA + gi);
+                        stcg(accA + gi, mk<T>(a.x + wA * p1 + wA2 * p2, a.y + wB * p1 + wB2 * p2));
+                    } else {
+                        const C pr = v[r] * zp;
+                        if (wA != (T)0) { const C a = ldcg(accA + gi); stcg(accA + gi, mk<T>(a.x + wA * pr.x, a.y + wA * pr.y)); }
+                        if (wB != (T)0) { const C a = ldcg(accB + gi); stcg(accB + gi, mk<T>(a.x + wB * pr.x, a.y + wB * pr.y)); }
+                    }
                 }
                 if (start) {
                     if (reload) e = ldcg(e4s + gbase + r * TPP * N * N);
-                    const C hb = v[r] * e;
+                    const C hb = cmul(v[r], e, cw);
                     L.st(ph + r * TPP * RB, hb);
-                    v[r] = hb * e;
+                    v[r] = cmul(hb, e, cw);
                 }
             }
             release(bA, true);                                          // q_s -> slice store
@@ -574,7 +581,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                 if (st == 0) {                                              // F = e2 Dz F;  H = Dz'[e2 Dz' H]
                     m2_wait(&b_full[bB], uB & 1, A.err);
 #pragma unroll
-                    for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + pen + VAc + r * TPP * ES); v[r] = v[r] * (e * e); }
+                    for (int r = 0; r < 16; ++r) { const C e = L.ld(pB + pen + VAc + r * TPP * ES); v[r] = cmul(v[r], cmul(e, e, cw), cw); }
                     if (jobh) { store = false; st = 1; need_load = false; } else run = false;
                 } else run = false;
             } else run = false;                                             // Y1: F = Dy F, H = Dy' H;  Y2: H = Dy' H

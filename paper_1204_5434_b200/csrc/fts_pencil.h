@@ -206,7 +206,7 @@ FTS_HD void tdft_reg(cplx<T> (&v)[NV], const cplx<T> (&zp)[NZ]) {
             constexpr int L = decltype(ll)::value, Rc = R >> (L - 1), half = Rc / 2, Q = L >= 2 ? (1 << (L - 2)) : 1;
             static_for<0, (1 << (L - 1))>([&](auto bb) {
                 constexpr int blk = decltype(bb)::value, E = bitrev(blk, L - 1);
-                constexpr bool MI = L >= 2 && E >= Q;
+                [[maybe_unused]] constexpr bool MI = L >= 2 && E >= Q;
                 if constexpr (TWISTED) {
                     const cplx<T> w = mul_c16<((E % Q) * 16) / (1 << L)>(zp[ilog2(R) - L]);
                     static_for<0, half>([&](auto ii) {

@@ -632,3 +632,58 @@ def test_filter_passes_at_long_pencils(B, oracle, grid):
     g.propagate(); o.propagate()
     for x, y in zip(g.operators(), o.operators()):
         assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+
+
+# ------------------------------------------------------------------------------------------------
+# N1: real-field fast path (option "real_fields"): q and q+ marched together as z = q + i q+
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("grid,Ns,fA", [((16, 16, 16), 20, 0.3), ((32, 32, 32), 12, 0.5), ((8, 32, 16), 10, 0.8), ((64, 64, 64), 8, 0.25),
+                                         ((128, 128, 128), 8, 0.5), ((1, 16, 64), 10, 0.4)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_real_fields_fast_path(B, oracle, grid, Ns, fA, precision):
+    """Real W+ and W- (SCFT): the packed march reproduces the (complex) oracle: Q, phi_A, phi_B, slices of q and of q+ (block
+    junction before, at and after the middle; ticket, per-phase-launch and TMA marches), both store layouts."""
+    cfg = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=Ns, fA=fA, complex_fields=False)
+    for store_both in (0, 1):
+        g, o = _pair(B, oracle, cfg, precision=precision, store_both=store_both)
+        g.set_option("real_fields", 1)
+        g.propagate(); o.propagate()
+        Qg, pa, pb = g.density_operators(); Qo, oa, ob = o.density_operators()
+        tq, tp = (1e-11, 1e-9) if precision == "f64" else (2e-4, 2e-4)
+        assert Qg.imag == 0.0 and abs(Qg - Qo) <= tq * abs(Qo), (Qg, Qo)
+        assert np.max(np.abs(pa.cpu().numpy() - oa)) <= tp and np.max(np.abs(pb.cpu().numpy() - ob)) <= tp
+        for which in (0, 1):
+            for j in (0, 1, Ns // 2, Ns) + ((Ns - 1,) if store_both else ()):
+                assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - o.get_slice(which, j))) <= tp, (which, j)
+        with pytest.raises(B.FtsError) as e:
+            g.cl_step(0.01, 0, 1, 0)
+        assert e.value.status == 2
+        g.set_option("real_fields", 0)                 # and back: the general path on the same context
+        g.propagate()
+        Q2, pa2, _ = g.density_operators()
+        assert abs(Q2 - Qo) <= tq * abs(Qo) and np.max(np.abs(pa2.cpu().numpy() - oa)) <= tp
+
+
+def test_real_fields_scft_trajectory_and_misuse(B, oracle):
+    """SCFT iterations (both Seidel variants) with the option set follow the oracle; complex fields are reported (FTS_EINVAL);
+    one-propagator models refuse the option (FTS_EUNSUPPORTED)."""
+    cfg = inputs.config2(grid=(16, 16, 16), Ns=20)
+    for seidel in (0, 1):
+        g, o = _pair(B, oracle, cfg)
+        g.set_option("real_fields", 1)
+        for it in range(5):
+            Hg, rg = g.scft_step(5.0, 5.0, seidel)
+            Ho, ro = o.scft_step(5.0, 5.0, seidel)
+            assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9, (seidel, it)
+        for x, y in zip(g.get_fields(), o.get_fields()):
+            assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    bad = inputs.small_diblock(grid=(16, 16, 16), Ns=10, fA=0.4, complex_fields=True)
+    g, _ = _pair(B, oracle, bad)
+    g.set_option("real_fields", 1)
+    with pytest.raises(B.FtsError) as e:
+        g.scft_step(1.0, 1.0, 0)
+    assert e.value.status == 1                         # FTS_EINVAL: the declaration was wrong
+    g1 = B.Fts((16, 16, 16), (4.0,) * 3, 8, "external")
+    with pytest.raises(B.FtsError) as e:
+        g1.set_option("real_fields", 1)
+    assert e.value.status == 6
