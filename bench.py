@@ -232,7 +232,8 @@ def run_gpu(args):
     opts = dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt)
     if kind == "scft" and "real_fields" not in opts:
         opts["real_fields"] = 1                     # SCFT fields are real: q and q+ share one packed march (N1)
-    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, options=opts, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, options=opts, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C,
+              store_both=1 if args.store == "full" else 0)
     host = [torch.from_numpy(np.ascontiguousarray(f)).to(cdt).pin_memory() for f in (cfg.f0, cfg.f1) if f is not None]
     devf = [h.to(dev) for h in host]
     back = [torch.empty_like(h).pin_memory() for h in host]
@@ -343,7 +344,7 @@ def run_gpu(args):
                               "frac_of_floor": t_hbm / t_step}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-           "config": config_dict(cfg, kind, prec, world, {"options": opts} if opts else None),
+           "config": config_dict(cfg, kind, prec, world, {"options": opts, "slice_store": args.store, "workspace_GB": round(g.workspace.numel() / 1e9, 2)}),
            "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
                                                                                       "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),
@@ -374,6 +375,9 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="fts_set_option (tuning experiments), e.g. --opt march=2")
+    ap.add_argument("--store", default="full", choices=["full", "mitm"],
+                    help="slice store: full = every slice kept, densities by one streaming pass (fastest on a 180 GB part, the default here); "
+                         "mitm = the library's default meet-in-the-middle store, densities accumulated inside the march (half the memory)")
     ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--budget", type=float, default=20.0, help=argparse.SUPPRESS)
     args = ap.parse_args()

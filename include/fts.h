@@ -71,6 +71,14 @@ fts_status fts_create(const int grid[3], const double cell[3], int Ns, const fts
                       void* workspace_dev, size_t workspace_bytes, fts_ctx** out);
 fts_status fts_destroy(fts_ctx* ctx);
 
+/* Chain architecture of the two-species melt model (linear multiblock copolymers use the same
+ * propagators): nblocks blocks listed from the s = 0 chain end, species[i] in {0 = A, 1 = B}, steps[i] contour steps
+ * (even, >= 2, summing to Ns; host arrays).  Replaces the default AB diblock (fA Ns steps of A, then B): e.g. an ABA
+ * triblock is species {0,1,0}.  q marches from s = 0, q+ from the far end; densities use Simpson's rule per block.
+ * The SCFT / CL updates keep the homopolymer Debye kernel of Eq. 11 as their linear-response estimate.
+ * FTS_EUNSUPPORTED for the one-species models.  Synchronises the device. */
+fts_status fts_set_blocks(fts_ctx* ctx, int nblocks, const int* species, const int* steps);
+
 /* Copy fields into / out of the context (device to device).  f1_dev is NULL for one-field models. */
 fts_status fts_set_fields(fts_ctx* ctx, const void* f0_dev, const void* f1_dev, void* stream);
 fts_status fts_get_fields(fts_ctx* ctx, void* f0_dev, void* f1_dev, void* stream);

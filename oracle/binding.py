@@ -30,6 +30,7 @@ def lib():
         L.oracle_propagate.argtypes = [vp]
         L.oracle_propagate_steps.argtypes = [vp, C.c_int]
         L.oracle_density_operators.argtypes = [vp, vp, vp, dp]
+        L.oracle_set_blocks.argtypes = [vp, C.c_int, ip, ip]
         L.oracle_get_slice.argtypes = [vp, C.c_int, C.c_int, vp]
         L.oracle_scft_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, dp, dp]
         L.oracle_cl_step.argtypes = [vp, C.c_double, C.c_int, C.c_uint64, C.c_uint64]
@@ -94,6 +95,10 @@ class Oracle:
         b = np.empty(self.grid, self.cdtype) if self.model == 2 else None
         self._chk(lib().oracle_get_fields(self.h, _ptr(a), _ptr(b)), "oracle_get_fields")
         return a, b
+
+    def set_blocks(self, species, steps):
+        n = len(species)
+        self._chk(lib().oracle_set_blocks(self.h, n, (C.c_int * n)(*species), (C.c_int * n)(*steps)), "oracle_set_blocks")
 
     def propagate(self, nsteps=None):
         if nsteps is None:

@@ -163,12 +163,17 @@ struct CtxBase {
     virtual int scft_step(double, double, int, double*, double*) = 0;
     virtual int cl_step(double, int, uint64_t, uint64_t) = 0;
     virtual int operators(double*, double*, double*) = 0;
+    virtual int set_blocks(int, const int*, const int*) = 0;
 };
 
 template <class T>
 struct Ctx : CtxBase {
     typedef std::complex<T> cx;
     int g[3]; double L[3]; int Ns; oracle_params P; size_t M; int jA; int nspecies;
+    // Chain architecture (linear multiblock copolymers use the same propagator machinery): blocks listed
+    // from the s = 0 end, each with a species (0 = A, 1 = B) and a number of contour steps.  Default: one block (homopolymer)
+    // or the AB diblock (jA steps of A, Ns - jA of B).
+    std::vector<std::pair<int, int>> blocks;
     std::vector<double> k2;
     std::vector<T> D1, Dh;                    // exp(-k^2 ds), exp(-k^2 ds/2)   (O1)
     std::vector<cx> f0, f1;                   // stored fields
@@ -181,6 +186,7 @@ struct Ctx : CtxBase {
         M = (size_t)g[0] * g[1] * g[2];
         nspecies = (P.model == 2) ? 2 : 1;
         jA = (P.model == 2) ? (int)std::lround(P.fA * Ns) : Ns;
+        if (P.model == 2) blocks = {{0, jA}, {1, Ns - jA}}; else blocks = {{0, Ns}};
         k2 = build_k2(g, L);
         const double ds = 1.0 / Ns;
         D1.resize(M); Dh.resize(M);
@@ -188,6 +194,30 @@ struct Ctx : CtxBase {
     }
 
     double V() const { return L[0] * L[1] * L[2]; }
+
+    // species of the contour segment [j, j+1]; Simpson weight of slice j in the density of species a (composite Simpson 1/3
+    // applied separately per block, reading A-5: a junction slice carries 1/3 from each block it bounds)
+    int seg_species(int j) const {
+        int s0 = 0;
+        for (auto& b : blocks) { if (j < s0 + b.second) return b.first; s0 += b.second; }
+        return blocks.back().first;
+    }
+    double block_weight(int a, int j) const {
+        double w = 0.0; int s0 = 0;
+        for (auto& b : blocks) { if (b.first == a) w += simpson_w(j, s0, s0 + b.second); s0 += b.second; }
+        return w;
+    }
+    int set_blocks(int n, const int* species, const int* steps) override {
+        if (P.model != 2) return 6;
+        if (n < 1 || !species || !steps) return 1;
+        int tot = 0;
+        for (int i = 0; i < n; ++i) { if ((species[i] != 0 && species[i] != 1) || steps[i] < 2 || (steps[i] & 1)) return 1; tot += steps[i]; }
+        if (tot != Ns) return 1;
+        blocks.clear();
+        for (int i = 0; i < n; ++i) blocks.push_back({species[i], steps[i]});
+        have_prop = false;
+        return 0;
+    }
 
     // O2: species fields from stored fields.
     std::vector<cx> species_field(int alpha) const {
@@ -246,16 +276,16 @@ struct Ctx : CtxBase {
         }
         q.assign(Ns + 1, std::vector<cx>());
         q[0].assign(M, cx(1, 0));                                  // q(x,0) = 1
-        for (int j = 0; j < nsteps; ++j) {                         // O5: species A for j < jA, else B
-            int a = (nspecies == 2 && j >= jA) ? 1 : 0;
+        for (int j = 0; j < nsteps; ++j) {                         // O5: the species of the block that segment [j, j+1] lies in
+            int a = (nspecies == 2) ? seg_species(j) : 0;
             step(e2[a], e4[a], q[j], q[j + 1]);
         }
         qd.clear();
         if (nspecies == 2) {                                       // O6: q+ indexed from the far end (reading A-2)
             qd.assign(Ns + 1, std::vector<cx>());
             qd[0].assign(M, cx(1, 0));                             // q+(x, s=1) = 1
-            for (int m = 0; m < nsteps; ++m) {
-                int a = (m < Ns - jA) ? 1 : 0;
+            for (int m = 0; m < nsteps; ++m) {                     // step m of q+ crosses the segment [Ns-m-1, Ns-m]
+                int a = seg_species(Ns - 1 - m);
                 step(e2[a], e4[a], qd[m], qd[m + 1]);
             }
         }
@@ -273,7 +303,7 @@ struct Ctx : CtxBase {
         const T ds = (T)(1.0 / Ns);
         phiA.assign(M, cx(0, 0)); phiB.assign(M, cx(0, 0));
         for (int j = 0; j <= Ns; ++j) {
-            T cA = (T)simpson_w(j, 0, jA), cB = (T)simpson_w(j, jA, Ns);
+            T cA = (T)block_weight(0, j), cB = (T)block_weight(1, j);
             const std::vector<cx>& a = q[j]; const std::vector<cx>& b = qdag(Ns - j);
             for (size_t i = 0; i < M; ++i) {
                 cx p = a[i] * b[i];
@@ -387,7 +417,7 @@ struct Ctx : CtxBase {
         // K = (ds/Q) sum_j c_j (1/M) sum_x q+_{Ns-j} F^-1{ -k^2 F{q_j} }
         cd K(0, 0);
         for (int j = 0; j <= Ns; ++j) {
-            double c = simpson_w(j, 0, jA) + ((nspecies == 2) ? simpson_w(j, jA, Ns) : 0.0);
+            double c = block_weight(0, j) + ((nspecies == 2) ? block_weight(1, j) : 0.0);
             std::vector<cx> lap = q[j];
             fft3d(lap, g, -1);
             for (size_t i = 0; i < M; ++i) lap[i] *= (T)(-k2[i]);
@@ -448,6 +478,7 @@ int oracle_set_fields(oracle_ctx* c, const void* a, const void* b) { return c ? 
 int oracle_get_fields(oracle_ctx* c, void* a, void* b) { return c ? c->impl->get_fields(a, b) : 1; }
 int oracle_propagate(oracle_ctx* c) { return c ? c->impl->propagate(-1) : 1; }
 int oracle_propagate_steps(oracle_ctx* c, int n) { return c ? c->impl->propagate(n) : 1; }
+int oracle_set_blocks(oracle_ctx* c, int n, const int* species, const int* steps) { return c ? c->impl->set_blocks(n, species, steps) : 1; }
 int oracle_density_operators(oracle_ctx* c, void* a, void* b, double Q[2]) { return c ? c->impl->density(a, b, Q) : 1; }
 int oracle_get_slice(oracle_ctx* c, int which, int j, void* out) { return c ? c->impl->get_slice(which, j, out) : 1; }
 int oracle_scft_step(oracle_ctx* c, double dp, double dm, int seidel, double H[2], double r[2]) { return c ? c->impl->scft_step(dp, dm, seidel, H, r) : 1; }

@@ -50,6 +50,9 @@ int  oracle_propagate(oracle_ctx*);
 /* march only the first nsteps contour steps (truncated parity at 256^3); Q is then mean(q_nsteps). */
 int  oracle_propagate_steps(oracle_ctx*, int nsteps);
 /* O8: phi_A, phi_B (Eq. 8, composite Simpson per block), Q. phiB may be NULL for one species. */
+/* Linear AB multiblock chain: blocks from the s = 0 end, species[i] in {0 = A, 1 = B}, steps[i] even, sum = Ns.
+ * Diblock model only (6 otherwise); replaces the default (fA Ns of A, then B).  Densities use Simpson's rule per block. */
+int  oracle_set_blocks(oracle_ctx*, int nblocks, const int* species, const int* steps);
 int  oracle_density_operators(oracle_ctx*, void* phiA, void* phiB, double Q_out[2]);
 int  oracle_get_slice(oracle_ctx*, int which, int j, void* out);
 int  oracle_scft_step(oracle_ctx*, double dt_plus, double dt_minus, int seidel, double H_out[2], double resid_out[2]);

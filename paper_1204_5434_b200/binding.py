@@ -15,7 +15,7 @@ STATUS = {0: "FTS_OK", 1: "FTS_EINVAL", 2: "FTS_ESTATE", 3: "FTS_EWORKSPACE", 4:
           6: "FTS_EUNSUPPORTED"}
 MODELS = {"external": 0, "edwards": 1, "diblock": 2}
 EXPORTS = ["fts_workspace_bytes", "fts_create", "fts_destroy", "fts_set_fields", "fts_get_fields", "fts_propagate",
-           "fts_propagate_steps", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
+           "fts_propagate_steps", "fts_set_blocks", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
            "fts_operators", "fts_set_option", "fts_debug_normals", "fts_debug_philox", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
 
 
@@ -45,6 +45,7 @@ def lib():
         L.fts_workspace_bytes.argtypes = [ip, C.c_int, pp, C.c_int, C.POINTER(C.c_size_t)]
         L.fts_create.argtypes = [ip, dp, C.c_int, pp, C.c_int, vp, C.c_size_t, C.POINTER(vp)]
         L.fts_destroy.argtypes = [vp]
+        L.fts_set_blocks.argtypes = [vp, C.c_int, ip, ip]
         L.fts_set_fields.argtypes = [vp, vp, vp, vp]
         L.fts_get_fields.argtypes = [vp, vp, vp, vp]
         L.fts_propagate.argtypes = [vp, vp]
@@ -115,6 +116,11 @@ class Fts:
     def set_option(self, key, value):
         with torch.cuda.device(self.device):
             self._chk(lib().fts_set_option(self.h, str(key).encode(), int(value)), f"fts_set_option({key})")
+
+    def set_blocks(self, species, steps):
+        n = len(species)
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_set_blocks(self.h, n, (C.c_int * n)(*[int(v) for v in species]), (C.c_int * n)(*[int(v) for v in steps])), "fts_set_blocks")
 
     def close(self):
         if getattr(self, "h", None) and _lib is not None:

@@ -28,6 +28,8 @@ struct Ctx {
     // workspace carve-up
     DimTables dim[3];
     double *cA, *cB, *scal, *kacc; double2* partial;
+    signed char* seg;             // device: species per contour segment
+    std::vector<int> blk_species, blk_steps;      // chain architecture: blocks from the s = 0 end (fts_set_blocks)
     void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2], *acc[2][2];
     int keep, nslots;             // slice store: slices 0..keep at slot s, the last slice of a march at slot keep + 1 (fts_march.cuh)
     bool have_fields, have_prop, have_phi; int marched;
@@ -52,7 +54,7 @@ enum { MARCH_MAXCHUNKS = 64 };
 static int counters_per_step(const int g[3]) { const int a = 2 + 2 * MARCH_MAXCHUNKS, b = 2 + 2 * g[0]; return a > b ? a : b; }
 
 struct Layout {          // the single place that decides where things live in the workspace
-    size_t off_tab[3][2], off_tw[3], off_tw2[3], off_k2[3], off_cA, off_cB, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
+    size_t off_tab[3][2], off_tw[3], off_tw2[3], off_k2[3], off_cA, off_cB, off_seg, off_scal, off_kacc, off_partial, off_phases, off_counters, counters_bytes;
     size_t off_f[2], off_e4[2], off_F[2], off_H[2], off_q[2], off_phi[2], off_G[2], off_acc[2][2], total; int keep, nslots;
 };
 static Layout make_layout(const int g[3], int Ns, int model, size_t esz, int store_both) {
@@ -67,6 +69,7 @@ static Layout make_layout(const int g[3], int Ns, int model, size_t esz, int sto
     }
     Lo.off_cA = o; o += align_up((size_t)(Ns + 1) * sizeof(double));
     Lo.off_cB = o; o += align_up((size_t)(Ns + 1) * sizeof(double));
+    Lo.off_seg = o; o += align_up((size_t)Ns + 1);
     Lo.off_scal = o; o += align_up(64 * sizeof(double));
     Lo.off_kacc = o; o += align_up((size_t)(Ns + 1) * 2 * sizeof(double));
     Lo.off_partial = o; o += align_up(1024 * sizeof(double2));
@@ -302,7 +305,8 @@ static const void* e4_field(const Ctx* c, int i) { return i < 2 ? c->e4[i] : (c-
 static DensArgs dens_args(const Ctx* c, int nsteps) {
     DensArgs D;
     for (int b = 0; b < 2; ++b) for (int a = 0; a < 2; ++a) D.acc[b][a] = c->acc[b][a];
-    D.cA = c->cA; D.cB = c->cB; D.on = nsteps == c->Ns; D.keep = c->keep; D.half = c->Ns / 2;
+    // accumulate inside the march only with the meet-in-the-middle store; a full store is summed by density_store_kernel afterwards
+    D.cA = c->cA; D.cB = c->cB; D.on = nsteps == c->Ns && c->keep != c->Ns; D.keep = c->keep; D.half = c->Ns / 2;
     return D;
 }
 
@@ -313,7 +317,7 @@ static void fill_march_args(const Ctx* c, MarchArgs& A, int nsteps) {
     for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
     A.nprop = c->nprop; A.packed = c->packed;
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; A.tw[d] = c->dim[d].tw; A.g[d] = c->g[d]; }
-    A.M = (long long)c->M; A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nsteps = nsteps;
+    A.M = (long long)c->M; A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nsteps = nsteps; A.seg = c->seg;
     A.done = c->counters; A.err = (int*)((char*)c->counters + c->counters_bytes - 128);
     A.dens = dens_args(c, nsteps);
 }
@@ -451,7 +455,7 @@ static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     March2Args A; std::memset(&A, 0, sizeof A);
     for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; }
     for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
-    A.packed = c->packed;
+    A.packed = c->packed; A.seg = c->seg;
     for (int d = 0; d < 3; ++d) { A.tab[d][0] = c->dim[d].tab[0]; A.tab[d][1] = c->dim[d].tab[1]; }
     A.tw = c->dim[0].tw2;
     A.Ns = c->Ns; A.jA = c->jA; A.nspecies = c->nspecies; A.nprop = c->nprop; A.nsteps = nsteps; A.lag = c->v2_lag; A.skew = c->v2_skew;
@@ -470,7 +474,7 @@ template <class T>
 static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     MarchArgs A; fill_march_args<T>(c, A, nsteps);
     CK(cudaMemsetAsync(c->counters, 0, c->counters_bytes - 128, st));          // counters and ticket; the error flag stays until fts_set_fields
-    if (nsteps == c->Ns)                                                        // S6: the density sums the T items accumulate into
+    if (nsteps == c->Ns && c->keep != c->Ns)                                    // S6: the density sums the T items accumulate into
         for (int b = 0; b < c->nprop; ++b) for (int a = 0; a < c->nspecies; ++a) CK(cudaMemsetAsync(c->acc[b][a], 0, c->M * c->esz, st));
     if (c->v2) return march2_t<T>(c, nsteps, st);
     if (c->persistent) {
@@ -540,6 +544,15 @@ static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
 // the march's T items.  Written to phiA / phiB (the context's own phi fields or the caller's).
 template <class T>
 static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
+    if (c->keep == c->Ns) {                                // full store: one streaming pass over the slices
+        const cplx<T>* q = (const cplx<T>*)c->q[0];
+        const cplx<T>* qd = (const cplx<T>*)c->q[c->nprop - 1];          // one propagator / packed: q+ lives in the same store
+        density_store_kernel<T><<<(unsigned)((c->M + 255) / 256), 256, 0, st>>>(q, qd, c->M, c->Ns, c->cA, c->cB, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA,
+                                                                                 c->nspecies == 2 ? (cplx<T>*)phiB : nullptr, c->packed);
+        g_launches += 1;
+        CK(cudaGetLastError());
+        return FTS_OK;
+    }
     if (c->packed) {
         density_finish_packed_kernel<T><<<ew_blocks(c->M), 256, 0, st>>>((const cplx<T>*)c->acc[0][0], (int)c->M, c->scal + S_Q, 1.0 / c->Ns, (cplx<T>*)phiA, (cplx<T>*)phiB);
         g_launches += 1;
@@ -733,6 +746,25 @@ static void fill_tw2(int N, std::vector<cplx<T>>& tw2) {
     }
 }
 
+// Chain architecture -> device tables: species per contour segment, and the Simpson weights of every slice in the density of
+// species A and B (composite Simpson 1/3 per block, reading A-5: a junction slice carries 1/3 from each block it bounds).
+static fts_status upload_blocks(Ctx* c) {
+    const int Ns = c->Ns;
+    std::vector<signed char> seg(Ns + 1, 0);
+    std::vector<double> wA(Ns + 1, 0.0), wB(Ns + 1, 0.0);
+    int s0 = 0;
+    for (size_t i = 0; i < c->blk_steps.size(); ++i) {
+        const int sp = c->blk_species[i], n = c->blk_steps[i];
+        for (int j = s0; j < s0 + n; ++j) seg[j] = (signed char)sp;
+        for (int j = 0; j <= Ns; ++j) (sp == 0 ? wA : wB)[j] += simpson_weight(j, s0, s0 + n);
+        s0 += n;
+    }
+    CK(cudaMemcpy(c->seg, seg.data(), seg.size(), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->cA, wA.data(), wA.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->cB, wB.data(), wB.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return FTS_OK;
+}
+
 // S1: everything that is computed once per simulation
 template <class T>
 static fts_status build_tables(Ctx* c) {
@@ -761,10 +793,7 @@ static fts_status build_tables(Ctx* c) {
         CK(cudaMemcpy(c->dim[d].tw2, tw2.data(), N * sizeof(cplx<T>), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dim[d].k2, k2.data(), N * sizeof(double), cudaMemcpyHostToDevice));
     }
-    std::vector<double> wA(c->Ns + 1), wB(c->Ns + 1);
-    for (int j = 0; j <= c->Ns; ++j) { wA[j] = simpson_weight(j, 0, c->jA); wB[j] = c->nspecies == 2 ? simpson_weight(j, c->jA, c->Ns) : 0.0; }
-    CK(cudaMemcpy(c->cA, wA.data(), wA.size() * sizeof(double), cudaMemcpyHostToDevice));
-    CK(cudaMemcpy(c->cB, wB.data(), wB.size() * sizeof(double), cudaMemcpyHostToDevice));
+    fts_status rb = upload_blocks(c); if (rb) return rb;
     CK(cudaMemset(c->scal, 0, 64 * sizeof(double)));
     CK(cudaMemset(c->counters, 0, c->counters_bytes));
     return FTS_OK;
@@ -814,12 +843,13 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     c->M = (size_t)grid[0] * grid[1] * grid[2];
     c->nprop = c->nspecies = (P->model == FTS_MODEL_DIBLOCK) ? 2 : 1;
     c->jA = (P->model == FTS_MODEL_DIBLOCK) ? (int)std::lround(P->fA * Ns) : Ns;
+    if (P->model == FTS_MODEL_DIBLOCK) { c->blk_species = {0, 1}; c->blk_steps = {c->jA, Ns - c->jA}; } else { c->blk_species = {0}; c->blk_steps = {Ns}; }
     c->ws = (char*)ws; c->ws_bytes = ws_bytes;
     for (int d = 0; d < 3; ++d) {
         c->dim[d].tab[0] = c->ws + Lo.off_tab[d][0]; c->dim[d].tab[1] = c->ws + Lo.off_tab[d][1];
         c->dim[d].tw = c->ws + Lo.off_tw[d]; c->dim[d].tw2 = c->ws + Lo.off_tw2[d]; c->dim[d].k2 = (double*)(c->ws + Lo.off_k2[d]);
     }
-    c->cA = (double*)(c->ws + Lo.off_cA); c->cB = (double*)(c->ws + Lo.off_cB);
+    c->cA = (double*)(c->ws + Lo.off_cA); c->cB = (double*)(c->ws + Lo.off_cB); c->seg = (signed char*)(c->ws + Lo.off_seg);
     c->scal = (double*)(c->ws + Lo.off_scal); c->kacc = (double*)(c->ws + Lo.off_kacc); c->partial = (double2*)(c->ws + Lo.off_partial);
     c->f0 = c->ws + Lo.off_f[0]; c->f1 = c->ws + Lo.off_f[1];
     for (int i = 0; i < 2; ++i) {
@@ -864,6 +894,23 @@ fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     c->occ = 0;
     fts_status rc = replan(c);
     if (rc) return rc;
+    CK(cudaDeviceSynchronize());
+    c->have_prop = false;
+    return FTS_OK;
+}
+
+fts_status fts_set_blocks(fts_ctx* c, int nblocks, const int* species, const int* steps) {
+    if (!c || nblocks < 1 || !species || !steps) return FTS_EINVAL;
+    if (c->P.model != FTS_MODEL_DIBLOCK) return FTS_EUNSUPPORTED;
+    int tot = 0;
+    for (int i = 0; i < nblocks; ++i) {
+        if ((species[i] != 0 && species[i] != 1) || steps[i] < 2 || (steps[i] & 1)) return FTS_EINVAL;      // reading A-5: even blocks (Simpson)
+        tot += steps[i];
+    }
+    if (tot != c->Ns) return FTS_EINVAL;
+    CK(cudaDeviceSynchronize());                           // no march may be reading the tables
+    c->blk_species.assign(species, species + nblocks); c->blk_steps.assign(steps, steps + nblocks);
+    fts_status rc = upload_blocks(c); if (rc) return rc;
     CK(cudaDeviceSynchronize());
     c->have_prop = false;
     return FTS_OK;

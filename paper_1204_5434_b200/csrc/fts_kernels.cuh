@@ -5,7 +5,8 @@
 //                   field-update filters — forward, 3-D multiplier, inverse.  Used by the SCFT / Eq. 11 updates and Pi.
 // boltzmann_kernel  exp(-w ds/4) per species.
 // reduce_kernel     deterministic two-level sums / max (Q of Eq. 4, H of Eq. 2-3, residuals).
-// density_finish    phi = (ds/Q) x the Simpson sums the march accumulated (Eq. 8).
+// density_finish    phi = (ds/Q) x the Simpson sums the march accumulated (Eq. 8); density_store: the same
+//                   sums in one streaming pass over a full slice store (store_both = 1).
 // update kernels    forces of PAPER.md:84, Euler-Maruyama / semi-implicit updates of Eq. 9-11, Philox noise.
 #ifndef FTS_KERNELS_CUH
 #define FTS_KERNELS_CUH
@@ -268,6 +269,30 @@ __global__ void __launch_bounds__(1024) reduce_final_kernel(const double2* parti
 // items (fts_march.cuh DensArgs: meet-in-the-middle, one sum per propagator and species); this kernel adds the two
 // propagators' sums and multiplies by ds / Q.
 // ------------------------------------------------------------------------------------------------
+// The same sums from a FULL slice store (store_both = 1): one streaming pass over the 2 (Ns + 1) slices, fp64 accumulators.
+// On a 180 GB part this is the faster layout (the march then carries no density work): HBM-bound,
+// (2 (Ns + 1) + 2) E M bytes.  packed: z_j = q_j + i q+_j in one store, product Re z_j Im z_{Ns-j} (real).
+template <class T>
+__global__ void __launch_bounds__(256) density_store_kernel(const cplx<T>* q, const cplx<T>* qd, size_t M, int Ns, const double* cA, const double* cB,
+                                                            const double* Qdev, double ds, cplx<T>* phiA, cplx<T>* phiB, int packed) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    double ax = 0, ay = 0, bx = 0, by = 0;
+#pragma unroll 4
+    for (int j = 0; j <= Ns; ++j) {
+        const cplx<T> u = q[(size_t)j * M + i], w = qd[(size_t)(Ns - j) * M + i];
+        double px, py;
+        if (packed) { px = (double)u.x * (double)w.y; py = 0.0; }
+        else { px = (double)u.x * (double)w.x - (double)u.y * (double)w.y; py = (double)u.x * (double)w.y + (double)u.y * (double)w.x; }
+        const double wa = cA[j], wb = cB[j];
+        ax += wa * px; ay += wa * py;
+        bx += wb * px; by += wb * py;
+    }
+    const double qx = Qdev[0], qy = Qdev[1], den = ds / (qx * qx + qy * qy);     // multiply by ds * conj(Q)/|Q|^2
+    phiA[i] = mk<T>((T)((ax * qx + ay * qy) * den), (T)((ay * qx - ax * qy) * den));
+    if (phiB) phiB[i] = mk<T>((T)((bx * qx + by * qy) * den), (T)((by * qx - bx * qy) * den));
+}
+
 template <class T>
 __global__ void density_finish_kernel(const cplx<T>* a0, const cplx<T>* a1, const cplx<T>* b0, const cplx<T>* b1, int M, const double* Qdev, double ds,
                                       cplx<T>* phiA, cplx<T>* phiB) {

@@ -63,9 +63,12 @@ __host__ __device__ inline int slice_slot(int s, int keep) { return s <= keep ? 
 // share one complex march of z = q + i q+:  the Boltzmann multiplies act component-wise, (Re z e_q, Im z e_q+), with the
 // factor field packed as (exp(-w_{alpha(s)} ds/4), exp(-w_{alpha+(s)} ds/4)) for the species pair of step s.  Half the
 // transforms, half the slices.  species_index() names the factor field of a step; cmul() is the multiply of either mode.
-__host__ __device__ inline int species_index(int packed, int nspecies, int jA, int Ns, int b, int step) {
+// seg[j] = species of the contour segment [j, j+1] (linear multiblock chains; default: the AB diblock).
+// Step s of q crosses segment s; step m of q+ (indexed from the far end, reading A-2) crosses segment Ns - 1 - m.
+__device__ __forceinline__ int species_index(int packed, int nspecies, const signed char* seg, int Ns, int b, int step) {
     if (nspecies != 2) return 0;
-    const int sq = step >= jA ? 1 : 0, sqd = step < Ns - jA ? 1 : 0;       // O5 / O6 block schedule of q and of q+
+    step = step < 0 ? 0 : (step > Ns - 1 ? Ns - 1 : step);
+    const int sq = seg[step], sqd = seg[Ns - 1 - step];                     // O5 / O6 block schedule of q and of q+
     if (packed) return 2 * sq + sqd;
     return b == 0 ? sq : sqd;
 }
@@ -81,6 +84,7 @@ struct MarchArgs {
     int g[3];
     long long M;
     int Ns, jA, nspecies, nsteps;
+    const signed char* seg;     // species per contour segment (species_index)
     int nprop;                  // propagators marched (2 = diblock q and q+; 1 otherwise, and in packed mode)
     int packed;                 // N1 real-field fast path: ONE complex march of z = q + i q+ (see cmul_mode)
     int nchunks, planes;        // x-slabs and planes per slab
@@ -390,7 +394,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         cp_async_commit();
     };
     // species of contour step `step` of propagator b (O5 / O6 block schedule)
-    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.jA, A.Ns, b, step); };
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.seg, A.Ns, b, step); };
     const bool cw = A.packed != 0;
 
     int cur_dim = -1;
@@ -471,28 +475,53 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
 #pragma unroll
             for (int r = 0; r < EPT; ++r) {
                 const int i = c.base0 + r * c.estride;
-                C e = mk<T>(0, 0);
                 if (combine) {                                        // q_s = (4 e4 Dx'[H] - F)/3     (Eq. 12)
-                    e = s_stash[r * NT + tid];
+                    const C e = s_stash[r * NT + tid];
                     const C f = s_pre[r * NT + tid];
                     const C h = cmul(v[r], e, cw);
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                 }
                 if (c.active && keep) stcg(qs + i, v[r]);             // the slice store IS the step's output write
-                if (dens && c.active) {                               // Eq. 8: this slice times the stored partner, weighted, into the sums
-                    const C zp = self ? v[r] : ldcg(partner + i);
-                    if (cw) {                                         // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
-                        const T p1 = v[r].x * zp.y, p2 = zp.x * v[r].y;
-                        const C a = ldcg(accA + i);
-                        stcg(accA + i, mk<T>(a.x + (T)wA * p1 + (T)wA2 * p2, a.y + (T)wB * p1 + (T)wB2 * p2));
-                    } else {
-                        const C pr = v[r] * zp;
-                        if (wA != 0.0) { const C a = ldcg(accA + i); stcg(accA + i, mk<T>(a.x + (T)wA * pr.x, a.y + (T)wA * pr.y)); }
-                        if (wB != 0.0) { const C a = ldcg(accB + i); stcg(accB + i, mk<T>(a.x + (T)wB * pr.x, a.y + (T)wB * pr.y)); }
+            }
+            if (dens && c.active) {
+                // Eq. 8: this slice times the stored partner, weighted, into the sums.  All loads of a batch are issued before its
+                // first store (the compiler cannot hoist them itself: the stores might alias), so a batch costs ONE round trip.
+                constexpr int BATCH = EPT < (sizeof(T) == 8 ? 4 : 8) ? EPT : (sizeof(T) == 8 ? 4 : 8);
+                for (int pass = 0; pass < 2; ++pass) {                // species A, then B (both only at the block junction)
+                    const double w1 = pass == 0 ? wA : wB;
+                    if (cw ? pass == 1 : w1 == 0.0) continue;
+                    C* acc = cw ? accA : (pass == 0 ? accA : accB);
+#pragma unroll
+                    for (int r0 = 0; r0 < EPT; r0 += BATCH) {
+                        C zp[BATCH], a[BATCH];
+#pragma unroll
+                        for (int k = 0; k < BATCH; ++k) {
+                            const int i = c.base0 + (r0 + k) * c.estride;
+                            zp[k] = self ? v[r0 + k] : ldcg(partner + i);
+                            a[k] = ldcg(acc + i);
+                        }
+#pragma unroll
+                        for (int k = 0; k < BATCH; ++k) {
+                            const int i = c.base0 + (r0 + k) * c.estride;
+                            const C q = v[r0 + k];
+                            if (cw) {                                 // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
+                                const T p1 = q.x * zp[k].y, p2 = zp[k].x * q.y;
+                                stcg(acc + i, mk<T>(a[k].x + (T)wA * p1 + (T)wA2 * p2, a[k].y + (T)wB * p1 + (T)wB2 * p2));
+                            } else {
+                                const C pr = q * zp[k];
+                                stcg(acc + i, mk<T>(a[k].x + (T)w1 * pr.x, a[k].y + (T)w1 * pr.y));
+                            }
+                        }
                     }
                 }
-                if (start) {
+            }
+            if (start) {
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) {
+                    const int i = c.base0 + r * c.estride;
+                    C e;
                     if (reload) e = c.active ? ldcg(e4s + i) : mk<T>(0, 0);
+                    else e = s_stash[r * NT + tid];
                     const C hb = cmul(v[r], e, cw);
                     s_stash[r * NT + tid] = hb;
                     v[r] = cmul(hb, e, cw);

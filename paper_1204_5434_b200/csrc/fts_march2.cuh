@@ -48,6 +48,7 @@ struct March2Args {
     const void* tab[3][2];       // per dimension: exp(-k_d^2 ds)/N, exp(-k_d^2 ds/2)/N
     const void* tw;              // twiddles of the twisted second stage, tw2[slot * R1 + k1] (fts_pencil.h)
     int Ns, jA, nspecies, nprop, nsteps, lag, skew;
+    const signed char* seg;      // species per contour segment (fts_march.cuh, species_index)
     int packed;                  // N1 real-field fast path: one march of z = q + i q+ (fts_march.cuh, cmul)
     const void* q[2];            // slice stores (the density partner is read straight from global memory)
     DensArgs dens;               // S6: Simpson density sums accumulated by the T items (fts_march.cuh)
@@ -288,7 +289,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
     __syncthreads();
 
     const M2Sched<T, N> sched(A.nprop, A.lag, A.skew, A.nsteps);
-    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.jA, A.Ns, b, step); };      // O5 / O6 block schedule
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.seg, A.Ns, b, step); };      // O5 / O6 block schedule
     const bool cw = A.packed != 0;
     auto nbuf_of = [](int kind) { return kind == PH_T ? 3 : (kind == PH_Z ? 2 : 1); };
     // TMA coordinates of sub-tile g of a strided item (c0 in scalars), and the byte offset of a z item inside a field
@@ -494,6 +495,66 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
         C v[16];
         // q_s = (4 e4 Dx'[H] - F)/3 -> slice (Eq. 12);  start of step s: stash e4 q_s, v = e4^2 q_s.
         // Buffers of a T item: A = H (then q_s), B = e4 (then F), C = F (then the stash, then H).
+        // element r of this thread inside a field (x tiles): gbase_of() + r TPP N^2
+        auto gbase_of = [&]() {
+            const int tile = dv->idx * Cfg::G + w / Cfg::WPT, z = (tile % (N / 8)) * 8 + (w % Cfg::WPT) * Cfg::ZPW + zz, iy = tile / (N / 8);
+            return (t * N + iy) * N + z;
+        };
+        // S6 (Eq. 8, DensArgs): the slice just formed (re-read from the tile at pq) times the stored partner slice,
+        // Simpson-weighted, into the sums.  Partner and sums are read straight from global memory (prefetched into L2 when the
+        // item started), four elements per round trip: all loads of a batch are issued before its first store.
+        auto accumulate_density = [&](const unsigned char* pq) {
+            const int b = dv->b, s = dv->s; const bool two = A.nprop == 2;
+            const int jp = (two && b == 1) ? A.Ns - s : s;
+            const bool self = !two && s == A.dens.half;
+            T wA = (T)A.dens.cA[jp], wB = (T)A.dens.cB[jp], wA2 = 0, wB2 = 0;
+            if (cw) { if (!self) { wA2 = (T)A.dens.cA[A.Ns - jp]; wB2 = (T)A.dens.cB[A.Ns - jp]; } }
+            else if (!two && !self) wA += (T)A.dens.cA[A.Ns - jp];
+            const int gb = gbase_of();
+            const C* partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N + gb;
+            for (int pass = 0; pass < 2; ++pass) {                      // sums of species A, then B (both only at the block junction)
+                const T w1 = pass == 0 ? wA : wB, w2 = pass == 0 ? wA2 : wB2;
+                if (cw ? pass == 1 : w1 == (T)0) continue;
+                C* acc = static_cast<C*>(A.dens.acc[b][cw ? 0 : pass]) + gb;
+#pragma unroll 1
+                for (int r0 = 0; r0 < 16; r0 += 4) {
+                    C zp[4], a[4], q[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int off = (r0 + k) * TPP * N * N;
+                        q[k] = L.ld(pq + (r0 + k) * TPP * RB);
+                        zp[k] = self ? q[k] : ldcg(partner + off);
+                        a[k] = ldcg(acc + off);
+                    }
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int off = (r0 + k) * TPP * N * N;
+                        if (cw) {                                       // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
+                            const T p1 = q[k].x * zp[k].y, p2 = zp[k].x * q[k].y;
+                            stcg(acc + off, mk<T>(a[k].x + wA * p1 + wA2 * p2, a[k].y + wB * p1 + wB2 * p2));
+                        } else {
+                            const C pr = q[k] * zp[k];
+                            stcg(acc + off, mk<T>(a[k].x + w1 * pr.x, a[k].y + w1 * pr.y));
+                        }
+                    }
+                }
+                (void)w2;
+            }
+        };
+        // L2 prefetch of what accumulate_density will read (issued when the item starts, a transform ahead of its use)
+        auto prefetch_density = [&]() {
+            if ((zz & 1) != 0) return;
+            const int b = dv->b, s = dv->s; const bool two = A.nprop == 2;
+            const int gb = gbase_of();
+            const C* partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N + gb;
+            const int jp = (two && b == 1) ? A.Ns - s : s;
+            const C* acc = static_cast<const C*>(A.dens.acc[b][(cw || A.dens.cA[jp] != 0.0) ? 0 : 1]) + gb;
+#pragma unroll 4
+            for (int r = 0; r < 16; ++r) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(partner + r * TPP * N * N));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(acc + r * TPP * N * N));
+            }
+        };
         auto combine = [&]() {
             m2_wait(&b_full[bB], uB & 1, A.err);
             m2_wait(&b_full[bC], uC & 1, A.err);
@@ -502,25 +563,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
             unsigned char* pq = pA + sub + VAs; unsigned char* ph = pC + sub + VAs;
             const bool dens = flags & M2_DENS;
             const C* e4s = nullptr; int gbase = 0;
-            if (reload || dens) {                                       // element r of this thread inside a field: gbase + r TPP N^2
-                const int idx = dv->idx;
-                const int tile = idx * Cfg::G + w / Cfg::WPT, z = (tile % (N / 8)) * 8 + (w % Cfg::WPT) * Cfg::ZPW + zz, iy = tile / (N / 8);
-                gbase = (t * N + iy) * N + z;
-            }
-            if (reload) e4s = static_cast<const C*>(A.e4[dv->spS]);     // block junction: the new species' factors straight from global memory
-            // S6 (Eq. 8, DensArgs): this slice times the stored partner slice, Simpson-weighted, into the sums
-            const C* partner = nullptr; C* accA = nullptr; C* accB = nullptr; T wA = 0, wB = 0, wA2 = 0, wB2 = 0; bool self = false;
-            if (dens) {
-                const int b = dv->b, s = dv->s; const bool two = A.nprop == 2;
-                const int jp = (two && b == 1) ? A.Ns - s : s;
-                self = !two && s == A.dens.half;
-                double a = A.dens.cA[jp]; const double bb = A.dens.cB[jp];
-                if (cw) { if (!self) { wA2 = (T)A.dens.cA[A.Ns - jp]; wB2 = (T)A.dens.cB[A.Ns - jp]; } }
-                else if (!two && !self) a += A.dens.cA[A.Ns - jp];
-                wA = (T)a; wB = (T)bb;
-                partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N;
-                accA = static_cast<C*>(A.dens.acc[b][0]); accB = static_cast<C*>(A.dens.acc[b][1]);
-            }
+            if (reload) { gbase = gbase_of(); e4s = static_cast<const C*>(A.e4[dv->spS]); }      // block junction: the new species' factors straight from global memory
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
                 C e = L.ld(pe + r * TPP * RB);
@@ -530,19 +573,6 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                     v[r] = mk<T>(((T)4 * h.x - f.x) * (T)(1.0 / 3.0), ((T)4 * h.y - f.y) * (T)(1.0 / 3.0));
                 } else v[r] = mk<T>(1, cw ? 1 : 0);                              // q(x,0) = 1, q+(x,s=1) = 1
                 L.st(pq + r * TPP * RB, v[r]);
-                if (dens) {
-                    const int gi = gbase + r * TPP * N * N;
-                    const C zp = self ? v[r] : ldcg(partner + gi);
-                    if (cw) {                                           // z = q + i q+: pairs (s, Ns-s) and (Ns-s, s); sums (A, B) as (re, im)
-                        const T p1 = v[r].x * zp.y, p2 = zp.x * v[r].y;
-                        const C a = ldcg(accA + gi);
-                        stcg(accA + gi, mk<T>(a.x + wA * p1 + wA2 * p2, a.y + wB * p1 + wB2 * p2));
-                    } else {
-                        const C pr = v[r] * zp;
-                        if (wA != (T)0) { const C a = ldcg(accA + gi); stcg(accA + gi, mk<T>(a.x + wA * pr.x, a.y + wA * pr.y)); }
-                        if (wB != (T)0) { const C a = ldcg(accB + gi); stcg(accB + gi, mk<T>(a.x + wB * pr.x, a.y + wB * pr.y)); }
-                    }
-                }
                 if (start) {
                     if (reload) e = ldcg(e4s + gbase + r * TPP * N * N);
                     const C hb = cmul(v[r], e, cw);
@@ -550,10 +580,12 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                     v[r] = cmul(hb, e, cw);
                 }
             }
+            if (dens) accumulate_density(pq);
             release(bA, true);                                          // q_s -> slice store
             if (!start) { release(bB, false); release(bC, false); }
             return start;
         };
+        if (kind == PH_T && (flags & M2_DENS)) prefetch_density();
         m2_wait(&b_full[bA], uA & 1, A.err);
         unsigned char* cur = pA; int curb = bA;
         const T* tab = (kind == PH_T || jobh) ? tabd + N : tabd;

@@ -386,13 +386,15 @@ def test_config5_truncated_march_and_invariants(B, oracle_cfg5_first8, precision
         assert abs(Qj - Q) <= rel * abs(Q), j
     assert abs(complex(pa.to(torch.complex128).mean().item()) - cfg.fA) <= rel
     assert abs(complex((pa + pb).to(torch.complex128).mean().item()) - 1.0) <= rel
-    # the default (meet-in-the-middle) store gives the same Q and densities bit for bit: the arithmetic does not depend on it
+    # the default (meet-in-the-middle) store, densities accumulated inside the march, gives the same Q bit for bit and the same
+    # densities to rounding (the full store is summed in one pass with fp64 accumulators, in a different order)
     del g
     g2 = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
     g2.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
     g2.propagate()
     Q2, pa2, pb2 = g2.density_operators()
-    assert Q2 == Q and torch.equal(pa2, pa) and torch.equal(pb2, pb)
+    assert Q2 == Q
+    assert float((pa2 - pa).abs().max()) <= (1e-13 if precision == "f64" else 1e-5) and float((pb2 - pb).abs().max()) <= (1e-13 if precision == "f64" else 1e-5)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -687,3 +689,37 @@ def test_real_fields_scft_trajectory_and_misuse(B, oracle):
     with pytest.raises(B.FtsError) as e:
         g1.set_option("real_fields", 1)
     assert e.value.status == 6
+
+
+# ------------------------------------------------------------------------------------------------
+# N3: linear multiblock chains (fts_set_blocks)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("grid,Ns,blocks", [((16, 16, 16), 12, ([0, 1, 0], [2, 6, 4])), ((32, 32, 32), 16, ([1, 0, 1, 0], [2, 4, 6, 4])),
+                                             ((8, 32, 16), 10, ([0, 1, 0], [4, 4, 2])), ((128, 128, 128), 8, ([0, 1, 0], [2, 4, 2])),
+                                             ((64, 1, 1), 20, ([1, 0, 1], [6, 10, 4]))])
+@pytest.mark.parametrize("store_both", [0, 1])
+def test_multiblock_chains(B, oracle, grid, Ns, blocks, store_both):
+    """ABA and ABAB chains through every march (ticket, per-phase launches, TMA), both store layouts, complex fields; then
+    the real-field fast path on real fields; one SCFT iteration and one CL step follow the oracle with the same blocks."""
+    fA = 0.5 if Ns % 4 == 0 else 0.4                   # the default diblock the context is created with must itself be valid
+    cfg = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=Ns, fA=fA)
+    g, o = _pair(B, oracle, cfg, store_both=store_both)
+    g.set_blocks(*blocks); o.set_blocks(*blocks)
+    _cmp_solve(g, o, 1e-11, 1e-9, True)
+    for which in (0, 1):
+        for j in (1, Ns // 2, Ns):
+            assert np.max(np.abs(g.get_slice(which, j).cpu().numpy() - o.get_slice(which, j))) < 1e-9, (which, j)
+    if grid[0] <= 32:
+        Hg, rg = g.scft_step(2.0, 2.0, 1); Ho, ro = o.scft_step(2.0, 2.0, 1)
+        assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9
+        g.cl_step(0.01, 0, 3, 1); o.cl_step(0.01, 0, 3, 1)
+        for x, y in zip(g.get_fields(), o.get_fields()):
+            assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    real = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=Ns, fA=fA, complex_fields=False)
+    g, o = _pair(B, oracle, real, store_both=store_both)
+    g.set_blocks(*blocks); o.set_blocks(*blocks)
+    g.set_option("real_fields", 1)
+    _cmp_solve(g, o, 1e-11, 1e-9, True)
+    with pytest.raises(B.FtsError) as e:
+        g.set_blocks([0, 1], [3, Ns - 3])
+    assert e.value.status == 1

@@ -472,3 +472,51 @@ def test_create_rejects_bad_arguments(oracle):
         oracle.Oracle((4, 4, 4), (1.0,) * 3, 10, "diblock", fA=0.5)      # odd block (Simpson, reading A-5)
     with pytest.raises(ValueError):
         oracle.Oracle((4, 4, 4), (1.0,) * 3, 7, "external")
+
+
+# ------------------------------------------------------------------------------------------------
+# linear multiblock chains (oracle_set_blocks)
+# ------------------------------------------------------------------------------------------------
+def _solve_blocks(oracle, cfg, blocks=None, f0=None, f1=None, model="diblock"):
+    kw = dict(fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C)
+    o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, model, **kw)
+    if blocks is not None:
+        o.set_blocks(*blocks)
+    o.set_fields(cfg.f0 if f0 is None else f0, cfg.f1 if f1 is None else f1)
+    o.propagate()
+    return o, o.density_operators()
+
+
+def test_multiblock_pins(oracle):
+    """What fixes the block machinery without another implementation: (i) chain reversal - listing the blocks from the other
+    end swaps the roles of q and q+ and must leave Q, phi_A, phi_B unchanged (a wrong segment index for q+ breaks it);
+    (ii) two A blocks of even length are one homopolymer: Q and phi_A equal the one-species model in w_A = W+ - W-, phi_B = 0
+    (pins the junction weights 1/3 + 1/3 = 2/3 of Simpson per block, reading A-5); (iii) an ABA triblock obeys
+    mean q_j q+_{Ns-j} = Q for every j, mean phi_A = its A fraction and phi_A + phi_B averages to 1; in a uniform field
+    phi_A is identically that fraction; (iv) the two-block list reproduces the default diblock bit for bit."""
+    from paper_1204_5434_b200 import inputs
+    cfg = inputs.small_diblock(grid=(8, 4, 8), cell=(3.0, 4.0, 5.0), Ns=12, fA=0.5)
+    _, (Q0, a0, b0) = _solve_blocks(oracle, cfg)
+    _, (Q1, a1, b1) = _solve_blocks(oracle, cfg, ([0, 1], [6, 6]))
+    assert Q0 == Q1 and np.array_equal(a0, a1) and np.array_equal(b0, b1)                                  # (iv)
+    for blocks, rev in ((([0, 1], [4, 8]), ([1, 0], [8, 4])), (([0, 1, 0], [2, 6, 4]), ([0, 1, 0], [4, 6, 2])),
+                        (([1, 0, 1, 0], [2, 2, 4, 4]), ([0, 1, 0, 1], [4, 4, 2, 2]))):
+        _, (Qa, aa, ba) = _solve_blocks(oracle, cfg, blocks)
+        _, (Qb, ab, bb) = _solve_blocks(oracle, cfg, rev)
+        assert abs(Qa - Qb) < 1e-13 * abs(Qa) and np.max(np.abs(aa - ab)) < 1e-13 and np.max(np.abs(ba - bb)) < 1e-13      # (i)
+    _, (Qh, ah, bh) = _solve_blocks(oracle, cfg, ([0, 0], [4, 8]))                                          # (ii)
+    oe = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "external")
+    oe.set_fields(cfg.f0 - cfg.f1); oe.propagate()
+    Qe, ae, _ = oe.density_operators()
+    assert abs(Qh - Qe) < 1e-14 * abs(Qe) and np.max(np.abs(ah - ae)) < 1e-13 and np.max(np.abs(bh)) == 0.0
+    o, (Qt, at, bt) = _solve_blocks(oracle, cfg, ([0, 1, 0], [2, 6, 4]))                                    # (iii)
+    for j in range(cfg.Ns + 1):
+        assert abs(np.mean(o.get_slice(0, j) * o.get_slice(1, cfg.Ns - j)) - Qt) < 1e-13 * abs(Qt), j
+    assert abs(np.mean(at) - 0.5) < 1e-13 and abs(np.mean(at + bt) - 1.0) < 1e-13
+    w0 = 0.3 - 0.2j
+    _, (Qu, au, bu) = _solve_blocks(oracle, cfg, ([0, 1, 0], [2, 6, 4]), f0=np.full(cfg.grid, w0), f1=np.zeros(cfg.grid, complex))
+    assert abs(Qu - np.exp(-w0)) < 1e-14 and np.max(np.abs(au - 0.5)) < 1e-13 and np.max(np.abs(bu - 0.5)) < 1e-13
+    with pytest.raises(RuntimeError):
+        oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "diblock", fA=0.5).set_blocks([0, 1], [5, 7])             # odd blocks: no Simpson
+    with pytest.raises(RuntimeError):
+        oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, "external").set_blocks([0], [12])
