@@ -33,7 +33,7 @@
 namespace fts {
 
 enum { PH_T = 0, PH_Y1 = 1, PH_Z = 2, PH_Y2 = 3 };
-enum { MARCH_MAXPH = 512 };
+enum { MARCH_MAXPH = 512, MARCH_SEG_SMEM = 1024 };
 
 struct Phase {              // one entry of the round template ("round" j holds the phases listed in make_template)
     int first;              // first ticket of the phase inside the round
@@ -233,11 +233,15 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
     C* s_stash = s_x + Cfg::XELEMS;                        // thread-private [r][tid]: e4 tile, then the stashed half-branch input
     C* s_pre = s_stash + NT * EPT;                         // thread-private [r][tid]: primary input of the NEXT item (and F of a T item)
     Phase* s_ph = reinterpret_cast<Phase*>(s_pre + NT * EPT);
+    __shared__ signed char s_seg[MARCH_SEG_SMEM];      // species per contour segment (a global load per lookup would sit on every item's critical path)
     __shared__ int s_item[R][4];              // step, phase index, index inside the phase, state (0: end of march, 1: work)
     __shared__ __align__(8) uint64_t s_full[R], s_done[R];
 
     const int tid = threadIdx.x;
     for (int i = tid; i < A.nphases; i += Cfg::LAUNCH) s_ph[i] = A.phases[i];
+    const bool seg_in_smem = A.Ns <= MARCH_SEG_SMEM;
+    if (seg_in_smem && A.nspecies == 2) for (int i = tid; i < A.Ns; i += Cfg::LAUNCH) s_seg[i] = A.seg[i];
+    const signed char* const seg = seg_in_smem ? s_seg : A.seg;
     if (tid == 0) {
         for (int i = 0; i < R; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_done[i], NT); }
     }
@@ -394,7 +398,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         cp_async_commit();
     };
     // species of contour step `step` of propagator b (O5 / O6 block schedule)
-    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.seg, A.Ns, b, step); };
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, seg, A.Ns, b, step); };
     const bool cw = A.packed != 0;
 
     int cur_dim = -1;

@@ -34,7 +34,7 @@
 
 namespace fts {
 
-enum { M2_NBUF = 3, M2_RING = 4, M2_NT = 128, M2_LAUNCH = 192 };
+enum { M2_NBUF = 3, M2_RING = 4, M2_NT = 128, M2_LAUNCH = 192, M2_SEG_SMEM = 224 };
 enum { M2_FIRST = 1, M2_FIN = 2, M2_START = 4, M2_RELOAD = 8, M2_JOBH = 16, M2_KEEP = 32, M2_DENS = 64 };
 enum { M2_MAP_F = 0, M2_MAP_H = 2, M2_MAP_E = 4, M2_MAP_Q = 8 };     // + propagator (F, H, Q) or factor-field index (E, 0..3)
 
@@ -83,6 +83,7 @@ struct M2Cfg {
     static constexpr int NY1 = 2 * NY, NZZ = 2 * NZ, NY2 = NY;
     static constexpr int C2 = 2 + 2 * N;                    // counters per (propagator, step)
     static constexpr size_t SMEM = (size_t)M2_NBUF * BUFB + (size_t)N * ES + (size_t)6 * N * sizeof(T) + 512;
+    static_assert(3 * M2_NBUF * 8 + 2 * M2_RING * 8 + M2_RING * 32 + M2_SEG_SMEM <= 512, "control block overflows");
     static_assert(S::G1 == 1 && TPP == R2 && G * TILEB == 2048 * ES && PPI * N * ES == 2048 * ES && BUFB % 1024 == 0, "unsupported shape");
 };
 
@@ -277,10 +278,15 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
     uint64_t* b_ifull = b_free + M2_NBUF;                            // [4] item descriptor published
     uint64_t* b_iempty = b_ifull + M2_RING;                          // [4] descriptor no longer needed (4 warps + store thread)
     M2Desc* s_desc = reinterpret_cast<M2Desc*>(b_iempty + M2_RING);  // [4]
+    signed char* s_seg = reinterpret_cast<signed char*>(s_desc + M2_RING);      // species per contour segment, for the producer's lookups; inside the 512-byte control block
+                                                                     // (complex128 at N = 256 fits two CTAs per SM with 0.5 KB to spare: no static shared memory)
 
     const int tid = threadIdx.x;
     for (int i = tid; i < N; i += M2_LAUNCH) s_tw[i] = static_cast<const C*>(A.tw)[i];      // tw2 layout (Pencil::fwd2_b), N/2 entries used
     for (int i = tid; i < 6 * N; i += M2_LAUNCH) s_tab[i] = static_cast<const T*>(A.tab[i / (2 * N)][(i / N) & 1])[i % N];
+    const bool seg_in_smem = A.Ns <= M2_SEG_SMEM;
+    if (seg_in_smem && A.nspecies == 2) for (int i = tid; i < A.Ns; i += M2_LAUNCH) s_seg[i] = A.seg[i];
+    const signed char* const seg = seg_in_smem ? s_seg : A.seg;
     if (tid == 0) {
         for (int i = 0; i < M2_NBUF; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_out[i], M2_NT); mbar_init(&b_free[i], 1); }
         for (int i = 0; i < M2_RING; ++i) { mbar_init(&b_ifull[i], 1); mbar_init(&b_iempty[i], 5); }
@@ -289,7 +295,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
     __syncthreads();
 
     const M2Sched<T, N> sched(A.nprop, A.lag, A.skew, A.nsteps);
-    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, A.seg, A.Ns, b, step); };      // O5 / O6 block schedule
+    auto species = [&](int b, int step) -> int { return species_index(A.packed, A.nspecies, seg, A.Ns, b, step); };      // O5 / O6 block schedule
     const bool cw = A.packed != 0;
     auto nbuf_of = [](int kind) { return kind == PH_T ? 3 : (kind == PH_Z ? 2 : 1); };
     // TMA coordinates of sub-tile g of a strided item (c0 in scalars), and the byte offset of a z item inside a field
