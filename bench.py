@@ -243,6 +243,8 @@ def run_gpu(args):
     def step(i):
         if kind == "cl":
             g.cl_step(cfg.dt, 0, seed, i)
+            if args.ops_every and i % args.ops_every == 0:      # operator sampling (config 4: <mu>, <Pi>): out of the step's own solve
+                g.operators(want_pi=args.store == "full")
         elif kind == "scft":
             g.scft_step(cfg.dt_scft[0], cfg.dt_scft[1], 1)
         else:
@@ -344,7 +346,7 @@ def run_gpu(args):
                               "frac_of_floor": t_hbm / t_step}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-           "config": config_dict(cfg, kind, prec, world, {"options": opts, "slice_store": args.store, "workspace_GB": round(g.workspace.numel() / 1e9, 2)}),
+           "config": config_dict(cfg, kind, prec, world, {"options": opts, "ops_every": args.ops_every, "slice_store": args.store, "workspace_GB": round(g.workspace.numel() / 1e9, 2)}),
            "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
                                                                                       "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),
@@ -378,6 +380,7 @@ def main():
     ap.add_argument("--store", default="full", choices=["full", "mitm"],
                     help="slice store: full = every slice kept, densities by one streaming pass (fastest on a 180 GB part, the default here); "
                          "mitm = the library's default meet-in-the-middle store, densities accumulated inside the march (half the memory)")
+    ap.add_argument("--ops-every", type=int, default=0, help="CL workloads: call fts_operators (H, mu, Pi) every K steps inside the timed region (0 = never)")
     ap.add_argument("--oracle-worker", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--budget", type=float, default=20.0, help=argparse.SUPPRESS)
     args = ap.parse_args()

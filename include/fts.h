@@ -114,7 +114,9 @@ fts_status fts_scft_step(fts_ctx* ctx, double dt_plus, double dt_minus, int seid
  * Box-Muller, variance 2 lambda dt / dV, generated inside the update kernel.  Asynchronous. */
 fts_status fts_cl_step(fts_ctx* ctx, double dt, int scheme, uint64_t seed, uint64_t step, void* stream);
 
-/* Operators of the current fields; needs a completed fts_propagate.  H: Eq. 2 (Edwards, extensive) or
+/* Operators of the current fields; needs a completed fts_propagate - or a preceding fts_cl_step, in which case the
+ * operators are those of the fields that step STARTED from, taken from the solve it already did (no further
+ * propagator solve: operator averages over a CL run cost two small reductions per sample).  H: Eq. 2 (Edwards, extensive) or
  * Eq. 3 / (CV) (diblock); mu = ln C - ln Q; Pi: volume derivative of ln Z at fixed lattice fields (derived in
  * DESIGN.md, not printed in the paper: secondary output; needs store_both = 1, FTS_ESTATE otherwise).  Any pointer may be
  * NULL.  Synchronises `stream`. */

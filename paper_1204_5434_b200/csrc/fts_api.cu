@@ -33,6 +33,7 @@ struct Ctx {
     void *f0, *f1, *e4[2], *F[2], *H[2], *q[2], *phi[2], *G[2], *acc[2][2];
     int keep, nslots;             // slice store: slices 0..keep at slot s, the last slice of a march at slot keep + 1 (fts_march.cuh)
     bool have_fields, have_prop, have_phi; int marched;
+    bool ops_entry;               // the last call was fts_cl_step: Q, the slices and the field sums of the fields it STARTED from are still there
     // march schedule (fts_march.cuh)
     Phase* phases;            // device: persistent template at [0], the four per-launch templates at [MARCH_MAXPH * (1..4)]
     unsigned* counters;       // device: completion counters, then ticket and error flag
@@ -536,7 +537,7 @@ static fts_status propagate_t(Ctx* c, int nsteps, cudaStream_t st) {
     const cplx<T>* qlast = (const cplx<T>*)c->q[0] + (size_t)slice_slot(nsteps, c->keep) * M;
     if (c->packed) CK((reduce<T, RED_SUMRE>(c, qlast, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st, flag)));      // z = q + i q+: Q = mean Re z
     else CK((reduce<T, RED_SUM>(c, qlast, nullptr, 0.0, 1.0 / (double)M, c->scal + S_Q, st, flag)));
-    c->marched = nsteps; c->have_prop = true; c->have_phi = false;
+    c->marched = nsteps; c->have_prop = true; c->have_phi = false; c->ops_entry = false;
     return FTS_OK;
 }
 
@@ -570,10 +571,11 @@ static fts_status density_t(Ctx* c, void* phiA, void* phiB, cudaStream_t st) {
 
 // F^-1{ filt(k^2) F{g} } in place: z and y forward passes, x pass with the 3-D multiplier, y and z inverse passes
 template <class T>
-static fts_status filter3d_t(Ctx* c, void* g, Filt f, cudaStream_t st) {
+static fts_status filter3d_t(Ctx* c, void* g, Filt f, cudaStream_t st, const void* src = nullptr) {      // src: read the field from there (g receives the result)
     PassArgs A; std::memset(&A, 0, sizeof A);
-    A.job[0] = mkjob(g, g, OP_FWD);
+    A.job[0] = mkjob(src ? src : g, g, OP_FWD);
     CK(launch_pass<T>(c, 2, A, 1, st));
+    A.job[0] = mkjob(g, g, OP_FWD);
     CK(launch_pass<T>(c, 1, A, 1, st));
     A.job[0] = mkjob(g, g, OP_FILT); A.filt = f;
     CK(launch_pass<T>(c, 0, A, 1, st));
@@ -626,11 +628,22 @@ static fts_status scft_step_t(Ctx* c, double dtp, double dtm, int seidel, double
     return FTS_OK;
 }
 
+// field parts of H: Edwards sum_x Omega^2 (Eq. 2), diblock mean_x [W-^2/chiN - W+] (Eq. 3)
+template <class T>
+static fts_status field_sums_t(Ctx* c, cudaStream_t st) {
+    if (c->P.model == FTS_MODEL_EDWARDS) CK((reduce<T, RED_SUMSQ>(c, c->f0, nullptr, 0.0, 1.0, c->scal + S_SQ, st)));
+    if (c->P.model == FTS_MODEL_DIBLOCK) CK((reduce<T, RED_DIBLOCK_H>(c, c->f0, c->f1, 1.0 / c->P.chiN, 1.0 / (double)c->M, c->scal + S_H, st)));
+    return FTS_OK;
+}
+
 template <class T>
 static fts_status cl_step_t(Ctx* c, double dt, int scheme, uint64_t seed, uint64_t step, cudaStream_t st) {
     const int M = (int)c->M; const int nb = ew_blocks(c->M);
     fts_status rc = propagate_t<T>(c, c->Ns, st); if (rc) return rc;
     rc = density_t<T>(c, c->phi[0], c->phi[1], st); if (rc) return rc;
+    // the operators of the fields this step starts from cost no further solve: keep their field sums (two small reductions);
+    // fts_operators after fts_cl_step then reports H, mu (and Pi) of those fields (config 4 averages them over the run)
+    rc = field_sums_t<T>(c, st); if (rc) return rc;
     const double dV = c->L[0] * c->L[1] * c->L[2] / (double)c->M;
     const double lp = c->P.lambda_plus, lm = c->P.lambda_minus, ns = c->P.noise_scale;
     if (c->P.model == FTS_MODEL_EDWARDS) {
@@ -659,7 +672,7 @@ static fts_status cl_step_t(Ctx* c, double dt, int scheme, uint64_t seed, uint64
         }
     }
     CK(cudaGetLastError());
-    c->have_prop = false;
+    c->have_prop = false; c->ops_entry = true;
     return FTS_OK;
 }
 
@@ -675,13 +688,11 @@ static fts_status operators_t(Ctx* c, double* Ho, double* muo, double* Pio, cuda
     if (Pio) {                                             // K_j = (1/M) sum_x q+_{Ns-j} Laplacian(q_j)
         Filt f; f.type = FILT_NEGK2; f.a = 1.0; f.b = f.c = 0.0;
         for (int j = 0; j <= Ns; ++j) {
-            CK(cudaMemcpyAsync(c->G[0], q + (size_t)j * M, M * sizeof(cplx<T>), cudaMemcpyDeviceToDevice, st));
-            rc = filter3d_t<T>(c, c->G[0], f, st); if (rc) return rc;
+            rc = filter3d_t<T>(c, c->G[0], f, st, q + (size_t)j * M); if (rc) return rc;      // the first pass reads the slice in place
             CK((reduce<T, RED_PROD>(c, c->G[0], qd + (size_t)(Ns - j) * M, 0.0, 1.0 / (double)M, c->kacc + 2 * j, st)));
         }
     }
-    if (c->P.model == FTS_MODEL_EDWARDS) CK((reduce<T, RED_SUMSQ>(c, c->f0, nullptr, 0.0, 1.0, c->scal + S_SQ, st)));
-    if (c->P.model == FTS_MODEL_DIBLOCK) CK((reduce<T, RED_DIBLOCK_H>(c, c->f0, c->f1, 1.0 / c->P.chiN, 1.0 / (double)M, c->scal + S_H, st)));
+    if (!c->ops_entry) { rc = field_sums_t<T>(c, st); if (rc) return rc; }      // after fts_cl_step: the sums of its entry fields are already there
     std::vector<double> kh(2 * (Ns + 1), 0.0);
     if (Pio) CK(cudaMemcpyAsync(kh.data(), c->kacc, kh.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
     double h[12];
@@ -859,7 +870,7 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     }
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->keep = Lo.keep; c->nslots = Lo.nslots;
-    c->have_fields = c->have_prop = c->have_phi = false; c->marched = 0; c->occ = 0;
+    c->have_fields = c->have_prop = c->have_phi = c->ops_entry = false; c->marched = 0; c->occ = 0;
     c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0;
     c->packed = 0;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
@@ -922,7 +933,7 @@ fts_status fts_set_fields(fts_ctx* c, const void* f0, const void* f1, void* stre
     CK(cudaMemcpyAsync(c->f0, f0, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
     if (c->P.model == FTS_MODEL_DIBLOCK) CK(cudaMemcpyAsync(c->f1, f1, c->M * c->esz, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync((char*)c->counters + c->counters_bytes - 128, 0, sizeof(int), st));      // new fields: clear a previous march's error flag
-    c->have_fields = true; c->have_prop = false;
+    c->have_fields = true; c->have_prop = false; c->ops_entry = false;
     return FTS_OK;
 }
 fts_status fts_get_fields(fts_ctx* c, void* f0, void* f1, void* stream) {
@@ -990,7 +1001,7 @@ fts_status fts_cl_step(fts_ctx* c, double dt, int scheme, uint64_t seed, uint64_
 
 fts_status fts_operators(fts_ctx* c, double H[2], double mu[2], double Pi[2], void* stream) {
     if (!c) return FTS_EINVAL;
-    if (!c->have_prop || c->marched != c->Ns) return FTS_ESTATE;
+    if (!(c->have_prop || c->ops_entry) || c->marched != c->Ns) return FTS_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     return DISPATCH(operators_t<double>(c, H, mu, Pi, st), operators_t<float>(c, H, mu, Pi, st));
 }

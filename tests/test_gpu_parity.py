@@ -723,3 +723,27 @@ def test_multiblock_chains(B, oracle, grid, Ns, blocks, store_both):
     with pytest.raises(B.FtsError) as e:
         g.set_blocks([0, 1], [3, Ns - 3])
     assert e.value.status == 1
+
+
+@pytest.mark.parametrize("model", ["edwards", "diblock"])
+def test_operators_of_the_cl_steps_entry_fields(B, oracle, model):
+    """Config 4's deliverable is <mu>, <Pi> over a CL run: fts_operators after fts_cl_step reports the operators of the fields
+    the step started from, out of the solve the step already did (no second solve).  Oracle: operators before its step."""
+    if model == "edwards":
+        cfg = inputs.config4(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10)
+    else:
+        cfg = inputs.small_diblock(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4, C=20.0)
+    g, o = _pair(B, oracle, cfg)
+    n0 = B.launch_count()
+    for step in range(3):
+        o.propagate(); ref = o.operators()
+        o.cl_step(0.01, 0, 5, step)
+        g.cl_step(0.01, 0, 5, step)
+        for x, y in zip(g.operators(), ref):
+            assert abs(x - y) < 1e-9 * max(1.0, abs(y)), step
+    with pytest.raises(B.FtsError):
+        g.get_slice(0, 1)                              # the slices belong to the previous fields: not served
+    g.propagate()
+    o.propagate()
+    for x, y in zip(g.operators(), o.operators()):
+        assert abs(x - y) < 1e-9 * max(1.0, abs(y))
