@@ -140,6 +140,18 @@ def config_dict(cfg, kind, prec, world, extra=None):
     return d
 
 
+def run_options(args, kind):
+    opts = dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt)
+    if kind == "scft" and "real_fields" not in opts:
+        opts["real_fields"] = 1                     # SCFT fields are real (PAPER.md:94-96): q and q+ share one packed march (N1)
+    return opts
+
+
+def run_extras(args, kind):
+    """config keys that name HOW the workload is run; identical in both arms (the oracle ignores them: it always keeps every slice)."""
+    return {"options": run_options(args, kind), "ops_every": args.ops_every, "slice_store": args.store}
+
+
 def oracle_host_aggregate(workload, budget_s, n_steps_hint):
     """BASELINE.md plan (ii): P independent oracle processes concurrently on the host's cores (no threading inside the oracle);
     P = the box's core count, capped by memory and at 32.  Returns (aggregate units/s, P, cpu_count, text)."""
@@ -187,7 +199,7 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * full_units / value, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": config_dict(cfg, kind, "f64", 1),
+        "data": "synthetic", "config": config_dict(cfg, kind, args.precision, max(1, args.gpus), run_extras(args, kind)),
         "note": "ms_per_step is the full step extrapolated from the bounded sample (the oracle's cost is linear in contour steps)",
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"per step: {what}"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -229,9 +241,7 @@ def run_gpu(args):
     cdt = torch.complex128 if prec == "f64" else torch.complex64
     M, nprop = int(np.prod(cfg.grid)), (2 if cfg.model == "diblock" else 1)
     E = 16 if prec == "f64" else 8
-    opts = dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt)
-    if kind == "scft" and "real_fields" not in opts:
-        opts["real_fields"] = 1                     # SCFT fields are real (PAPER.md:94-96): q and q+ share one packed march (N1)
+    opts = run_options(args, kind)
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, options=opts, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C,
               store_both=1 if args.store == "full" else 0)
     host = [torch.from_numpy(np.ascontiguousarray(f)).to(cdt).pin_memory() for f in (cfg.f0, cfg.f1) if f is not None]
@@ -339,14 +349,14 @@ def run_gpu(args):
                 "peak_kind": f"vector {prec} FMA chains measured in this run (nominal {FP64_NOMINAL_TFLOPS if prec == 'f64' else FP32_NOMINAL_TFLOPS:.1f})"}
     else:
         roof = {"bound": "hbm", "achieved": b_alg / t_step / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": t_hbm / t_step, "peak_kind": pk_kind}
-    roof.update({"traffic": traffic, "traffic_source": traffic_src, "kernel": "march2_kernel / march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve, densities accumulated in the T items)", "launches_per_march": pass_launches,
+    roof.update({"traffic": traffic, "traffic_source": traffic_src, "kernel": "march2_kernel (128^3, 256^3) / march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve" + (")" if args.store == "full" else ", densities accumulated in the T items)"), "launches_per_march": pass_launches,
                  "avg_launch_us": ms_march * 1e3 / pass_launches, "alg_flops_per_launch": f_alg * rq / pass_launches,
                  "alg_bytes_per_launch": b_alg * rq / pass_launches, "march_ms": ms_march, "march_launches_all_kernels": march_launches,
                  "hbm_view": {"achieved_GBs_algorithmic": b_alg / t_step / 1e9, "peak_GBs": pk["hbm_gbs"], "peak_kind": pk_kind,
                               "frac_of_floor": t_hbm / t_step}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-           "config": config_dict(cfg, kind, prec, world, {"options": opts, "ops_every": args.ops_every, "slice_store": args.store, "workspace_GB": round(g.workspace.numel() / 1e9, 2)}),
+           "config": config_dict(cfg, kind, prec, world, run_extras(args, kind)), "workspace_GB": round(g.workspace.numel() / 1e9, 2),
            "iterations_per_s": {"value": world * args.steps / (ms * 1e-3), "iteration": {"cl": "fts_cl_step (1 propagator solve)", "scft": "fts_scft_step, seidel=1 (2 propagator solves)",
                                                                                       "propagate": "fts_propagate + fts_density_operators"}[kind]},
            "clocks": clk.summary(),
