@@ -40,7 +40,10 @@ struct Ctx {
     size_t counters_bytes;
     int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
     // options (fts_set_option; no environment variables are read)
-    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields; } opt;
+    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields, graph; } opt;
+    // per-phase launch mode: the whole march (4 launches per step) captured once as a CUDA graph and replayed (launch-bound loop)
+    struct MarchGraph { cudaGraphExec_t exec; int nsteps; long long kernels; } graphs[2];
+    int ngraphs; cudaStream_t cap_stream;
     int packed;                   // N1 real-field fast path active: one march of z = q + i q+ (fts_march.cuh); nprop is then 1
     // TMA march for large cubic grids (fts_march2.cuh)
     int v2, v2_lag, v2_skew, v2_occ;
@@ -218,7 +221,16 @@ static cudaError_t launch_march_inst(const MarchArgs& A, int grid, bool query, M
         if (e != cudaSuccess) return e;
     }
     if (query) return cudaSuccess;
-    march_kernel<T, N, EPT, TZ><<<grid, Cfg::LAUNCH, Cfg::SMEM, st>>>(A);
+    if (A.ticket) march_kernel<T, N, EPT, TZ><<<grid, Cfg::LAUNCH, Cfg::SMEM, st>>>(A);
+    else {                                                 // per-phase launch: programmatic dependent launch (see the kernel's prologue)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(Cfg::LAUNCH); cfg.dynamicSmemBytes = Cfg::SMEM; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, march_kernel<T, N, EPT, TZ>, A);
+        if (e != cudaSuccess) return e;
+    }
     g_launches += 1;
     return cudaGetLastError();
 }
@@ -333,6 +345,11 @@ static fts_status plan_march(Ctx* c) {
     int dev = 0; CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
     c->persistent = (Nx == Ny && Ny == Nz) && c->opt.march != FTS_MARCH_LAUNCH;
+    // Automatic choice for small cubic grids, from measurement (B200, Ns = 100): graph-replayed per-phase launches beat the
+    // persistent ticket kernel at 32^3 (2.4 vs 3.2 ms per diblock solve) and for ONE propagator at 64^3 (3.7 vs 4.2 ms: with
+    // no second propagator to fill the dependency hops the kernel's polling costs more than a graph edge); the persistent
+    // kernel wins at 16^3 and for two propagators at 64^3 and above.
+    if (c->opt.march == FTS_MARCH_AUTO && c->opt.graph && (Nx == 32 || (Nx == 64 && c->nprop == 1))) c->persistent = 0;
     // slab size (optional): F and H of the slabs in flight must sit in L2 next to the streaming traffic
     const size_t plane = (size_t)Ny * Nz * c->esz;
     size_t target = ~(size_t)0;        // default: one slab.  Slabs cut HBM traffic from 17 to 13 E*M, but the march is not HBM-bound and
@@ -471,6 +488,30 @@ static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     return FTS_OK;
 }
 
+// Per-phase launch mode: one launch per phase kind and step (stream order replaces the completion counters).
+template <class T>
+static fts_status march_launches_t(Ctx* c, MarchArgs A, int nsteps, cudaStream_t st) {
+    static const int dim_of[4] = {0, 1, 2, 1};
+    for (int j = 0; j <= nsteps; ++j) {
+        for (int k = 0; k < 4; ++k) {
+            if (k != PH_T && j == nsteps) break;
+            A.round0 = A.round1 = j;
+            if (k == PH_T && c->nprop == 2 && A.dens.on && j == A.dens.half) {
+                // the middle of the chain: q+'s item multiplies q+_h with the slice q_h that q's item of the SAME step stores
+                // (DensArgs), so the two propagators' T phases cannot share a launch here
+                for (int b = 0; b < 2; ++b) {
+                    A.phases = c->phases + MARCH_MAXPH * (1 + k) + 2 + b; A.nphases = 1; A.tickets_per_round = c->cnt[k];
+                    CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
+                }
+                continue;
+            }
+            A.phases = c->phases + MARCH_MAXPH * (1 + k); A.nphases = c->nprop; A.tickets_per_round = c->nprop * c->cnt[k];
+            CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
+        }
+    }
+    return FTS_OK;
+}
+
 template <class T>
 static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     MarchArgs A; fill_march_args<T>(c, A, nsteps);
@@ -497,24 +538,30 @@ static fts_status march_t(Ctx* c, int nsteps, cudaStream_t st) {
     }
     A.nchunks = 1; A.planes = c->g[0]; A.ticket = nullptr;
     A.ntT = c->cnt[PH_T]; A.nY1 = c->cnt[PH_Y1]; A.nZ = c->cnt[PH_Z]; A.nY2 = c->cnt[PH_Y2];
-    static const int dim_of[4] = {0, 1, 2, 1};
-    for (int j = 0; j <= nsteps; ++j) {
-        for (int k = 0; k < 4; ++k) {
-            if (k != PH_T && j == nsteps) break;
-            A.round0 = A.round1 = j;
-            if (k == PH_T && c->nprop == 2 && A.dens.on && j == A.dens.half) {
-                // the middle of the chain: q+'s item multiplies q+_h with the slice q_h that q's item of the SAME step stores
-                // (DensArgs), so the two propagators' T phases cannot share a launch here
-                for (int b = 0; b < 2; ++b) {
-                    A.phases = c->phases + MARCH_MAXPH * (1 + k) + 2 + b; A.nphases = 1; A.tickets_per_round = c->cnt[k];
-                    CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
-                }
-                continue;
-            }
-            A.phases = c->phases + MARCH_MAXPH * (1 + k); A.nphases = c->nprop; A.tickets_per_round = c->nprop * c->cnt[k];
-            CK(launch_march<T>(c, c->g[dim_of[k]], A, A.tickets_per_round, false, nullptr, nullptr, st));
-        }
-    }
+    if (!c->opt.graph) return march_launches_t<T>(c, A, nsteps, st);
+    // Launch-bound inner loop (4 small kernels per contour step): captured once per (context, nsteps) on a private stream and
+    // replayed as one graph on the caller's stream (the caller's stream may be the legacy default stream, which cannot capture).
+    for (int i = 0; i < c->ngraphs; ++i)
+        if (c->graphs[i].nsteps == nsteps) { CK(cudaGraphLaunch(c->graphs[i].exec, st)); g_launches += c->graphs[i].kernels; return FTS_OK; }
+    if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+    const uint64_t l0 = g_launches;
+    CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    fts_status rc = march_launches_t<T>(c, A, nsteps, c->cap_stream);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) { c->err = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e); return FTS_ECUDA; }
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { c->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e); return FTS_ECUDA; }
+    int slot;                                                                 // two shapes are kept: the first seen (normally the full march) and the latest other
+    if (c->ngraphs < 2) slot = c->ngraphs++;
+    else { slot = 1; cudaGraphExecDestroy(c->graphs[1].exec); }
+    c->graphs[slot].exec = exec; c->graphs[slot].nsteps = nsteps; c->graphs[slot].kernels = (long long)(g_launches - l0);
+    g_launches = l0;                                                          // capturing launched nothing
+    CK(cudaGraphLaunch(exec, st));
+    g_launches += c->graphs[slot].kernels;
     return FTS_OK;
 }
 
@@ -810,7 +857,13 @@ static fts_status build_tables(Ctx* c) {
     return FTS_OK;
 }
 
+static void drop_graphs(Ctx* c) {
+    for (int i = 0; i < c->ngraphs; ++i) if (c->graphs[i].exec) cudaGraphExecDestroy(c->graphs[i].exec);
+    c->ngraphs = 0;
+}
+
 static fts_status replan(Ctx* c) {
+    drop_graphs(c);
     fts_status rc = c->prec == FTS_F64 ? plan_march<double>(c) : plan_march<float>(c);
     if (!rc) rc = c->prec == FTS_F64 ? plan_march2<double>(c) : plan_march2<float>(c);
     return rc;
@@ -871,7 +924,8 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->keep = Lo.keep; c->nslots = Lo.nslots;
     c->have_fields = c->have_prop = c->have_phi = c->ops_entry = false; c->marched = 0; c->occ = 0;
-    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0;
+    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0; c->opt.graph = 1;
+    c->ngraphs = 0; c->cap_stream = nullptr;
     c->packed = 0;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
     rc = DISPATCH(build_tables<double>(c), build_tables<float>(c));
@@ -882,7 +936,11 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     return FTS_OK;
 }
 
-fts_status fts_destroy(fts_ctx* c) { delete c; return FTS_OK; }
+fts_status fts_destroy(fts_ctx* c) {
+    if (c) { drop_graphs(c); if (c->cap_stream) cudaStreamDestroy(c->cap_stream); }
+    delete c;
+    return FTS_OK;
+}
 
 fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     if (!c || !key) return FTS_EINVAL;
@@ -893,6 +951,7 @@ fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     else if (!std::strcmp(key, "skew")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.skew = (int)value; }
     else if (!std::strcmp(key, "interleave")) c->opt.interleave = value != 0;
     else if (!std::strcmp(key, "tz")) { if (value != 0 && value != 8 && value != 16) return FTS_EINVAL; c->opt.tz = (int)value; }
+    else if (!std::strcmp(key, "graph")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.graph = (int)value; }
     else if (!std::strcmp(key, "real_fields")) {
         if (value != 0 && value != 1) return FTS_EINVAL;
         if (value && c->P.model != FTS_MODEL_DIBLOCK) return FTS_EUNSUPPORTED;      // one propagator: nothing to pack

@@ -248,6 +248,12 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
     const int C2 = 2 + 2 * A.nchunks;         // counters per (propagator, step)
     const unsigned total = (unsigned)((A.round1 - A.round0 + 1) * A.tickets_per_round);
     __syncthreads();
+    // Per-phase launch mode chains ~4 Ns tiny kernels: with programmatic dependent launch the next kernel's CTAs are scheduled
+    // and run the prologue above (constant tables only) while this one's last stores drain (the trigger is at the END of a
+    // CTA's work: triggered at the start, the waiting CTAs of the next phase crowd the SMs and a 32^3 march gets 20 % slower);
+    // everything below reads what the previous kernel wrote and therefore waits for its completion and memory flush here.
+    // (No-ops without the launch attribute.)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     if (tid >= NT) {
         // ================= scheduler warp: one thread draws tickets, resolves dependencies, signals completions =================
@@ -590,6 +596,7 @@ __global__ void __launch_bounds__(MarchCfg<T, N, EPT, TZ>::LAUNCH, MarchCfg<T, N
         cur_pref = nxt_pref;
     }
     cp_async_wait<0>();
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
 }  // namespace fts
