@@ -14,6 +14,7 @@
 #include "fts_kernels.cuh"
 #include "fts_march.cuh"
 #include "fts_march2.cuh"
+#include "fts_plane.cuh"
 
 namespace fts {
 
@@ -40,7 +41,7 @@ struct Ctx {
     size_t counters_bytes;
     int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
     // options (fts_set_option; no environment variables are read)
-    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields, graph; } opt;
+    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields, graph, plane; } opt;
     // per-phase launch mode: the whole march (4 launches per step) captured once as a CUDA graph and replayed (launch-bound loop)
     struct MarchGraph { cudaGraphExec_t exec; int nsteps; long long kernels; } graphs[2];
     int ngraphs; cudaStream_t cap_stream;
@@ -345,11 +346,12 @@ static fts_status plan_march(Ctx* c) {
     int dev = 0; CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
     c->persistent = (Nx == Ny && Ny == Nz) && c->opt.march != FTS_MARCH_LAUNCH;
-    // Automatic choice for small cubic grids, from measurement (B200, Ns = 100): graph-replayed per-phase launches beat the
-    // persistent ticket kernel at 32^3 (2.4 vs 3.2 ms per diblock solve) and for ONE propagator at 64^3 (3.7 vs 4.2 ms: with
-    // no second propagator to fill the dependency hops the kernel's polling costs more than a graph edge); the persistent
-    // kernel wins at 16^3 and for two propagators at 64^3 and above.
-    if (c->opt.march == FTS_MARCH_AUTO && c->opt.graph && (Nx == 32 || (Nx == 64 && c->nprop == 1))) c->persistent = 0;
+    // Automatic choice for small cubic grids, from measurement (B200, Ns = 100, per diblock solve): the per-phase launches,
+    // replayed as one CUDA graph with programmatic dependent launch and with Y1/Z/Y2 fused into one kernel per yz-plane
+    // (fts_plane.cuh: two kernels per step), beat the persistent ticket kernel at 16^3 (2.55 -> 1.38 ms), 32^3 (3.25 -> 1.35 ms)
+    // and 64^3 (5.19 -> 4.31 ms; one propagator 4.2 -> 2.5 ms): on these grids a step is bound by the latency of its
+    // dependency hops, and a graph edge costs less than a completion counter polled through L2.
+    if (c->opt.march == FTS_MARCH_AUTO && c->opt.graph && c->opt.plane && (Nx == 16 || Nx == 32 || Nx == 64)) c->persistent = 0;
     // slab size (optional): F and H of the slabs in flight must sit in L2 next to the streaming traffic
     const size_t plane = (size_t)Ny * Nz * c->esz;
     size_t target = ~(size_t)0;        // default: one slab.  Slabs cut HBM traffic from 17 to 13 E*M, but the march is not HBM-bound and
@@ -488,13 +490,48 @@ static fts_status march2_t(Ctx* c, int nsteps, cudaStream_t st) {
     return FTS_OK;
 }
 
+// Fused yz-plane kernel (fts_plane.cuh) for Ny = Nz = 16, 32 or 64: replaces the Y1, Z and Y2 launches of a step.
+template <class T, int N, int EPT>
+static cudaError_t launch_plane_inst(const PlaneArgs& A, int grid, cudaStream_t st) {
+    typedef PlaneCfg<T, N, EPT> Cfg;
+    cudaError_t e = cudaFuncSetAttribute(plane_kernel<T, N, EPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = Cfg::SMEM; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, plane_kernel<T, N, EPT>, A);
+    g_launches += 1;
+    return e;
+}
+static int plane_planes_per_cta(const Ctx* c) {           // 0: the plane kernel does not apply to this grid
+    const int N = c->g[1];
+    if (!c->opt.plane || c->g[2] != N || (N != 16 && N != 32 && N != 64)) return 0;
+    const int pl = N == 16 ? 8 : 1;
+    return c->g[0] % pl == 0 ? pl : 0;
+}
+template <class T>
+static cudaError_t launch_plane(const Ctx* c, int step, cudaStream_t st) {
+    PlaneArgs A; std::memset(&A, 0, sizeof A);
+    for (int b = 0; b < 2; ++b) { A.F[b] = c->F[b]; A.H[b] = c->H[b]; }
+    for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
+    for (int d = 0; d < 2; ++d) { A.tab[d][0] = c->dim[1 + d].tab[0]; A.tab[d][1] = c->dim[1 + d].tab[1]; A.tw[d] = c->dim[1 + d].tw; }
+    A.seg = c->seg; A.Nx = c->g[0]; A.Ns = c->Ns; A.nspecies = c->nspecies; A.nprop = c->nprop; A.packed = c->packed; A.step = step;
+    const int pl = plane_planes_per_cta(c), grid = c->nprop * 2 * (c->g[0] / pl);
+    if (c->g[1] == 64) return launch_plane_inst<T, 64, 8>(A, grid, st);
+    return c->g[1] == 16 ? launch_plane_inst<T, 16, 16>(A, grid, st) : launch_plane_inst<T, 32, 8>(A, grid, st);
+}
+
 // Per-phase launch mode: one launch per phase kind and step (stream order replaces the completion counters).
 template <class T>
 static fts_status march_launches_t(Ctx* c, MarchArgs A, int nsteps, cudaStream_t st) {
     static const int dim_of[4] = {0, 1, 2, 1};
+    const bool planes = plane_planes_per_cta(c) > 0;       // small yz-planes: Y1, Z, Y2 fused into one kernel per step
     for (int j = 0; j <= nsteps; ++j) {
         for (int k = 0; k < 4; ++k) {
             if (k != PH_T && j == nsteps) break;
+            if (k != PH_T && planes) { CK(launch_plane<T>(c, j, st)); break; }
             A.round0 = A.round1 = j;
             if (k == PH_T && c->nprop == 2 && A.dens.on && j == A.dens.half) {
                 // the middle of the chain: q+'s item multiplies q+_h with the slice q_h that q's item of the SAME step stores
@@ -924,7 +961,7 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->keep = Lo.keep; c->nslots = Lo.nslots;
     c->have_fields = c->have_prop = c->have_phi = c->ops_entry = false; c->marched = 0; c->occ = 0;
-    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0; c->opt.graph = 1;
+    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0; c->opt.graph = 1; c->opt.plane = 1;
     c->ngraphs = 0; c->cap_stream = nullptr;
     c->packed = 0;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
@@ -951,6 +988,7 @@ fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     else if (!std::strcmp(key, "skew")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.skew = (int)value; }
     else if (!std::strcmp(key, "interleave")) c->opt.interleave = value != 0;
     else if (!std::strcmp(key, "tz")) { if (value != 0 && value != 8 && value != 16) return FTS_EINVAL; c->opt.tz = (int)value; }
+    else if (!std::strcmp(key, "plane")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.plane = (int)value; }
     else if (!std::strcmp(key, "graph")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.graph = (int)value; }
     else if (!std::strcmp(key, "real_fields")) {
         if (value != 0 && value != 1) return FTS_EINVAL;

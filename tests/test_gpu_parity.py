@@ -226,12 +226,13 @@ def test_determinism(B):
 # ------------------------------------------------------------------------------------------------
 # the march schedules (persistent ticket kernel with L2 slabs, stream-ordered launches) and full-size runs
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("opts", [{}, {"march": 1}, {"slab_bytes": 65536}, {"slab_bytes": 32768, "lag": 3},
-                                  {"interleave": 0, "slab_bytes": 131072}, {"tz": 8}])
+@pytest.mark.parametrize("opts", [{}, {"march": 1}, {"march": 1, "plane": 0}, {"march": 1, "plane": 0, "graph": 0}, {"march": 2}, {"march": 2, "slab_bytes": 65536},
+                                  {"march": 2, "slab_bytes": 32768, "lag": 3}, {"march": 2, "interleave": 0, "slab_bytes": 131072}, {"march": 2, "tz": 8}])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_march_schedules_agree(B, oracle, opts, precision):
-    """Cubic 32^3 grid (the persistent ticket kernel's domain): one slab, 8 and 16 slabs with different pipeline lags, and the
-    one-launch-per-phase mode all reproduce the oracle; they are also bit-identical to each other (fts_set_option)."""
+    """Cubic 32^3 grid: the automatic choice (graph-replayed launches with the fused yz-plane kernel), the per-phase launches
+    with and without plane fusion and graph, the persistent ticket kernel with one slab, 8 and 16 slabs and different pipeline
+    lags all reproduce the oracle; they are also bit-identical to each other (fts_set_option)."""
     cfg = inputs.small_diblock(grid=(32, 32, 32), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
     ref, _ = _pair(B, oracle, cfg, precision=precision)
     ref.propagate()
@@ -747,3 +748,35 @@ def test_operators_of_the_cl_steps_entry_fields(B, oracle, model):
     o.propagate()
     for x, y in zip(g.operators(), o.operators()):
         assert abs(x - y) < 1e-9 * max(1.0, abs(y))
+
+
+def test_streams_contexts_and_lifecycle(B, oracle):
+    """Host-side robustness: work enqueued on a non-blocking side stream (the graph-replayed launch mode captures on a private
+    stream and replays on the caller's), two contexts used alternately, and contexts created and destroyed repeatedly
+    (graphs instantiated and released) all reproduce the default-stream result bit for bit."""
+    cfg = inputs.small_diblock(grid=(32, 32, 32), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4)
+    g, o = _pair(B, oracle, cfg, store_both=0)
+    _cmp_solve(g, o, 1e-11, 1e-9, True)
+    Q0, pa0, pb0 = g.density_operators()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        g2 = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", **_kw(cfg))
+        g2.set_fields(_dev(cfg.f0), _dev(cfg.f1))
+        for _ in range(3):
+            g2.propagate()
+        Q1, pa1, pb1 = g2.density_operators()
+    side.synchronize()
+    assert Q1 == Q0 and torch.equal(pa1, pa0) and torch.equal(pb1, pb0)
+    other = inputs.small_diblock(grid=(16, 16, 16), cell=(4.0, 4.0, 4.0), Ns=10, fA=0.4, seed=3)
+    h, oh = _pair(B, oracle, other, store_both=0)
+    for _ in range(3):                                 # alternate two contexts (each with its own graph)
+        g.propagate(); h.propagate()
+    oh.propagate()
+    Qh, _, _ = h.density_operators(); Qo, _, _ = oh.density_operators()
+    assert abs(Qh - Qo) < 1e-11 * abs(Qo) and g.density_operators()[0] == Q0
+    for rep in range(25):
+        t = B.Fts(cfg.grid, cfg.cell, cfg.Ns, "diblock", **_kw(cfg))
+        t.set_fields(_dev(cfg.f0), _dev(cfg.f1))
+        t.propagate(4); t.propagate()
+        assert t.density_operators()[0] == Q0, rep
+        t.close()
