@@ -133,13 +133,14 @@ fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], 
  *   "interleave"  mode 2: alternate the two propagators' phases (default 1)
  *   "tz"          modes 1-2: pencils per strided tile, 8 or 16 (0 = default)
  *   "graph"       mode 1: replay the march's launches as one CUDA graph, captured once per context (default 1)
+ *   "tline"       mode 1: straight-line kernel for the x pass of a step when Nx <= 64 (default 1)
  *   "plane"       mode 1: fuse the y and z passes of a step into one kernel per yz-plane when Ny = Nz = 16 or 32 (default 1)
  *   "real_fields" 1: the caller declares that W+ and W- are real (SCFT; diblock only).  q and q+ are then
  *                 real and are marched together as ONE complex propagator z = q + i q+ (half the transforms and slices);
  *                 results agree with the general path to rounding; phi and slices are returned with zero imaginary part.
  *                 Fields that are not real make the next call that returns host scalars fail with FTS_EINVAL;
  *                 fts_cl_step (complex fields) is FTS_ESTATE and Pi FTS_EUNSUPPORTED while the option is set.
- * The march modes give bit-identical results among the ticket variants and agree to rounding with the TMA kernel. */
+ * The march modes agree to rounding (the ticket kernel's variants are bit-identical among themselves). */
 typedef enum { FTS_MARCH_AUTO = 0, FTS_MARCH_LAUNCH = 1, FTS_MARCH_TICKET = 2, FTS_MARCH_TMA = 3 } fts_march_mode;
 fts_status fts_set_option(fts_ctx* ctx, const char* key, long long value);
 

@@ -41,7 +41,7 @@ struct Ctx {
     size_t counters_bytes;
     int persistent, planes, nchunks, lag, nph, tickets_per_round, cnt[4], sms, occ;
     // options (fts_set_option; no environment variables are read)
-    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields, graph, plane; } opt;
+    struct { int march; long long slab_bytes; int lag, interleave, tz, skew, real_fields, graph, plane, tline; } opt;
     // per-phase launch mode: the whole march (4 launches per step) captured once as a CUDA graph and replayed (launch-bound loop)
     struct MarchGraph { cudaGraphExec_t exec; int nsteps; long long kernels; } graphs[2];
     int ngraphs; cudaStream_t cap_stream;
@@ -523,16 +523,58 @@ static cudaError_t launch_plane(const Ctx* c, int step, cudaStream_t st) {
     return c->g[1] == 16 ? launch_plane_inst<T, 16, 16>(A, grid, st) : launch_plane_inst<T, 32, 8>(A, grid, st);
 }
 
+// Straight-line T kernel (fts_plane.cuh) for x pencils of up to 64 points: replaces march_kernel's T launch of a step.
+template <class T, int N, int EPT>
+static cudaError_t launch_tline_inst(const TlineArgs& A, cudaStream_t st) {
+    typedef TlineCfg<T, N, EPT> Cfg;
+    cudaError_t e = cudaFuncSetAttribute(tline_kernel<T, N, EPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    const int ntile = A.plane / Cfg::TZ, items = (ntile + Cfg::GPB_S - 1) / Cfg::GPB_S;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(A.nb * items); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = Cfg::SMEM; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, tline_kernel<T, N, EPT>, A);
+    g_launches += 1;
+    return e;
+}
+static bool tline_ok(const Ctx* c) { const int N = c->g[0]; return c->opt.tline && (N == 1 || N == 8 || N == 16 || N == 32 || N == 64) && c->g[2] % 8 == 0; }
+template <class T>
+static cudaError_t launch_tline(const Ctx* c, const MarchArgs& M, int step, int b0, int nb, cudaStream_t st) {
+    TlineArgs A; std::memset(&A, 0, sizeof A);
+    for (int b = 0; b < 2; ++b) { A.q[b] = c->q[b]; A.F[b] = c->F[b]; A.H[b] = c->H[b]; }
+    for (int i = 0; i < 4; ++i) A.e4[i] = e4_field(c, i);
+    A.tab[0] = c->dim[0].tab[0]; A.tab[1] = c->dim[0].tab[1]; A.tw = c->dim[0].tw;
+    A.seg = c->seg; A.M = (long long)c->M; A.plane = c->g[1] * c->g[2];
+    A.Ns = c->Ns; A.nspecies = c->nspecies; A.nprop = c->nprop; A.packed = c->packed; A.step = step; A.nsteps = M.nsteps;
+    A.b0 = b0; A.nb = nb; A.dens = M.dens;
+    switch (c->g[0]) {
+        case 1: return launch_tline_inst<T, 1, 1>(A, st);
+        case 8: return launch_tline_inst<T, 8, 8>(A, st);
+        case 16: return launch_tline_inst<T, 16, 16>(A, st);
+        case 32: return launch_tline_inst<T, 32, 8>(A, st);
+        case 64: return launch_tline_inst<T, 64, 8>(A, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
 // Per-phase launch mode: one launch per phase kind and step (stream order replaces the completion counters).
 template <class T>
 static fts_status march_launches_t(Ctx* c, MarchArgs A, int nsteps, cudaStream_t st) {
     static const int dim_of[4] = {0, 1, 2, 1};
     const bool planes = plane_planes_per_cta(c) > 0;       // small yz-planes: Y1, Z, Y2 fused into one kernel per step
+    const bool tline = tline_ok(c);
     for (int j = 0; j <= nsteps; ++j) {
         for (int k = 0; k < 4; ++k) {
             if (k != PH_T && j == nsteps) break;
             if (k != PH_T && planes) { CK(launch_plane<T>(c, j, st)); break; }
             A.round0 = A.round1 = j;
+            if (k == PH_T && tline) {                      // straight-line T kernel; split per propagator at the middle of the chain (see below)
+                if (c->nprop == 2 && A.dens.on && j == A.dens.half) { CK(launch_tline<T>(c, A, j, 0, 1, st)); CK(launch_tline<T>(c, A, j, 1, 1, st)); }
+                else CK(launch_tline<T>(c, A, j, 0, c->nprop, st));
+                continue;
+            }
             if (k == PH_T && c->nprop == 2 && A.dens.on && j == A.dens.half) {
                 // the middle of the chain: q+'s item multiplies q+_h with the slice q_h that q's item of the SAME step stores
                 // (DensArgs), so the two propagators' T phases cannot share a launch here
@@ -961,7 +1003,7 @@ fts_status fts_create(const int grid_user[3], const double cell_user[3], int Ns,
     c->phases = (Phase*)(c->ws + Lo.off_phases); c->counters = (unsigned*)(c->ws + Lo.off_counters); c->counters_bytes = Lo.counters_bytes;
     c->keep = Lo.keep; c->nslots = Lo.nslots;
     c->have_fields = c->have_prop = c->have_phi = c->ops_entry = false; c->marched = 0; c->occ = 0;
-    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0; c->opt.graph = 1; c->opt.plane = 1;
+    c->opt.march = FTS_MARCH_AUTO; c->opt.slab_bytes = 0; c->opt.lag = -1; c->opt.interleave = 1; c->opt.tz = 0; c->opt.skew = -1; c->opt.real_fields = 0; c->opt.graph = 1; c->opt.plane = 1; c->opt.tline = 1;
     c->ngraphs = 0; c->cap_stream = nullptr;
     c->packed = 0;
     c->v2 = 0; c->v2_lag = c->v2_skew = c->v2_occ = 0;
@@ -988,6 +1030,7 @@ fts_status fts_set_option(fts_ctx* c, const char* key, long long value) {
     else if (!std::strcmp(key, "skew")) { if (value < -1 || value > 64) return FTS_EINVAL; c->opt.skew = (int)value; }
     else if (!std::strcmp(key, "interleave")) c->opt.interleave = value != 0;
     else if (!std::strcmp(key, "tz")) { if (value != 0 && value != 8 && value != 16) return FTS_EINVAL; c->opt.tz = (int)value; }
+    else if (!std::strcmp(key, "tline")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.tline = (int)value; }
     else if (!std::strcmp(key, "plane")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.plane = (int)value; }
     else if (!std::strcmp(key, "graph")) { if (value != 0 && value != 1) return FTS_EINVAL; c->opt.graph = (int)value; }
     else if (!std::strcmp(key, "real_fields")) {

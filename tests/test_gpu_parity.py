@@ -226,7 +226,7 @@ def test_determinism(B):
 # ------------------------------------------------------------------------------------------------
 # the march schedules (persistent ticket kernel with L2 slabs, stream-ordered launches) and full-size runs
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("opts", [{}, {"march": 1}, {"march": 1, "plane": 0}, {"march": 1, "plane": 0, "graph": 0}, {"march": 2}, {"march": 2, "slab_bytes": 65536},
+@pytest.mark.parametrize("opts", [{}, {"march": 1}, {"march": 1, "plane": 0}, {"march": 1, "tline": 0}, {"march": 1, "plane": 0, "graph": 0, "tline": 0}, {"march": 2}, {"march": 2, "slab_bytes": 65536},
                                   {"march": 2, "slab_bytes": 32768, "lag": 3}, {"march": 2, "interleave": 0, "slab_bytes": 131072}, {"march": 2, "tz": 8}])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_march_schedules_agree(B, oracle, opts, precision):
