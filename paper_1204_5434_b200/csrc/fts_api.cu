@@ -531,7 +531,7 @@ static cudaError_t launch_tline_inst(const TlineArgs& A, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     const int ntile = A.plane / Cfg::TZ, items = (ntile + Cfg::GPB_S - 1) / Cfg::GPB_S;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(A.nb * items); cfg.blockDim = dim3(Cfg::NT); cfg.dynamicSmemBytes = Cfg::SMEM; cfg.stream = st;
+    cfg.gridDim = dim3(A.nb * items); cfg.blockDim = dim3(Cfg::LAUNCH); cfg.dynamicSmemBytes = Cfg::SMEM; cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;

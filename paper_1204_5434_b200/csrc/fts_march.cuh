@@ -137,7 +137,7 @@ struct MarchCfg {
 };
 
 // barrier among the NT compute threads of a CTA (the scheduler warp does not take part)
-template <int NT> __device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); }
+template <int NT, int ID = 1> __device__ __forceinline__ void bar_compute() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NT) : "memory"); }
 
 // mbarrier primitives (shared memory, CTA scope): the scheduler warp and the compute warps hand items back and forth
 __device__ __forceinline__ void mbar_init(uint64_t* b, unsigned count) {
@@ -171,14 +171,14 @@ __device__ __forceinline__ bool mbar_wait(uint64_t* b, unsigned parity) {
 // exp(a ds d^2/dx_d^2) along the pencil: forward transform, real table (1/N folded in), inverse transform.
 // One shared-memory buffer serves both exchanges: every thread overwrites only what it last read.  `contig`
 // (block-uniform) selects the exchange addressing of the z pass (LC) or of the x/y passes (LS); the butterflies are shared.
-template <class T, int N, int EPT, int NT, class LS, class LC>
+template <class T, int N, int EPT, int NT, class LS, class LC, int BAR = 1>
 __device__ __forceinline__ void diffuse(cplx<T> (&v)[EPT], int t, int p, bool contig, const cplx<T>* s_tw, const T* tab, cplx<T>* xs, cplx<T>* xc) {
     typedef Pencil<T, N, EPT> P;
     typedef PencilShape<N, EPT> S;
     P::fwd_a(v, t, s_tw);
     if constexpr (!S::ONE) {
         if (contig) P::template xchg_store_a<LC>(v, t, xc, p); else P::template xchg_store_a<LS>(v, t, xs, p);
-        bar_compute<NT>();
+        bar_compute<NT, BAR>();
         if (contig) P::template xchg_load_b<LC>(v, t, xc, p); else P::template xchg_load_b<LS>(v, t, xs, p);
     }
     P::fwd_b(v);
@@ -187,7 +187,7 @@ __device__ __forceinline__ void diffuse(cplx<T> (&v)[EPT], int t, int p, bool co
     P::inv_b(v);
     if constexpr (!S::ONE) {
         if (contig) P::template xchg_store_b<LC>(v, t, xc, p); else P::template xchg_store_b<LS>(v, t, xs, p);
-        bar_compute<NT>();
+        bar_compute<NT, BAR>();
         if (contig) P::template xchg_load_a<LC>(v, t, xc, p); else P::template xchg_load_a<LS>(v, t, xs, p);
     }
     P::inv_a(v, t, s_tw);

@@ -117,8 +117,10 @@ __global__ void __launch_bounds__(PlaneCfg<T, N, EPT>::NT) plane_kernel(const Pl
 // march_kernel serves the same item through its scheduler warp, descriptor ring and staging buffers - machinery a kernel
 // that processes exactly one item per CTA does not need; on small grids, where a step is a chain of two few-microsecond
 // kernels, that overhead is a third of the T kernel.  Same butterflies, tables and arithmetic order: bit-identical results.
-// One CTA = 128 threads = GPB_S tiles [N x][8 z]; blockIdx.x -> (propagator, tile group).  The per-phase launch at the
-// middle of the chain is split per propagator by the host (q+'s item reads the slice q's item of the same step stores).
+// One CTA = GPB_S tiles [N x][8 z]; blockIdx.x -> (propagator, tile group).  SPLIT: a second group of 128 threads takes the
+// half branch (it receives e4 q_s through shared memory and runs Dx' while the first group runs Dx on e2 q_s), so the item's
+// critical path is two diffusions instead of three.  The per-phase launch at the middle of the chain is split per
+// propagator by the host (q+'s item reads the slice q's item of the same step stores).
 // ------------------------------------------------------------------------------------------------
 struct TlineArgs {
     void* q[2]; void* F[2]; void* H[2]; const void* e4[4];
@@ -140,11 +142,13 @@ struct TlineCfg {
     static constexpr int XELEMS = S::ONE ? 1 : GPB_S * N * TZ;
     typedef XchgLayout<1, S::R2 * TZ, TZ> LS;
     typedef XchgLayout<1, S::R2 + 1, 1> LC;                 // unused (strided layout only)
-    static constexpr size_t SMEM = (size_t)(N + XELEMS + NT * EPT) * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T);
+    static constexpr bool SPLIT = N == 64;                   // measured: 64^3 one propagator 2.13 -> 1.93 ms; no gain at 32, a loss at 16 (ONE-thread pencils)
+    static constexpr int LAUNCH = SPLIT ? 2 * NT : NT;
+    static constexpr size_t SMEM = (size_t)(N + (SPLIT ? 2 : 1) * XELEMS + NT * EPT) * sizeof(cplx<T>) + 2 * (size_t)N * sizeof(T);
 };
 
 template <class T, int N, int EPT>
-__global__ void __launch_bounds__(128) tline_kernel(const TlineArgs A) {
+__global__ void __launch_bounds__(TlineCfg<T, N, EPT>::LAUNCH, TlineCfg<T, N, EPT>::SPLIT ? 2 : 1) tline_kernel(const TlineArgs A) {
     typedef TlineCfg<T, N, EPT> Cfg;
     typedef typename Cfg::S S;
     typedef cplx<T> C;
@@ -154,11 +158,11 @@ __global__ void __launch_bounds__(128) tline_kernel(const TlineArgs A) {
     C* s_tw = reinterpret_cast<C*>(smem_raw);
     T* s_tab = reinterpret_cast<T*>(s_tw + N);                 // [full, half][N]
     C* s_x = reinterpret_cast<C*>(s_tab + 2 * N);              // exchange buffer of the transforms
-    C* s_stash = s_x + Cfg::XELEMS;                            // thread-private [r][tid]: the half-branch input e4 q_s
+    C* s_stash = s_x + (Cfg::SPLIT ? 2 : 1) * Cfg::XELEMS;     // [r][tid]: the half-branch input e4 q_s
 
-    const int tid = threadIdx.x;
-    for (int i = tid; i < N; i += NT) s_tw[i] = static_cast<const C*>(A.tw)[i];
-    for (int i = tid; i < 2 * N; i += NT) s_tab[i] = static_cast<const T*>(A.tab[i / N])[i % N];
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;  // group 1 (SPLIT): the half branch of the step that starts
+    for (int i = threadIdx.x; i < N; i += Cfg::LAUNCH) s_tw[i] = static_cast<const C*>(A.tw)[i];
+    for (int i = threadIdx.x; i < 2 * N; i += Cfg::LAUNCH) s_tab[i] = static_cast<const T*>(A.tab[i / N])[i % N];
     const int ntile = A.plane / TZ, items = (ntile + Cfg::GPB_S - 1) / Cfg::GPB_S;
     const int b = A.b0 + blockIdx.x / items, idx = blockIdx.x % items, s = A.step;
     const int sp_now = species_index(A.packed, A.nspecies, A.seg, A.Ns, b, s), sp_prev = species_index(A.packed, A.nspecies, A.seg, A.Ns, b, s - 1);
@@ -179,9 +183,24 @@ __global__ void __launch_bounds__(128) tline_kernel(const TlineArgs A) {
     const int tile = idx * Cfg::GPB_S + tb;
     const bool active = tile < ntile;
     const long long base0 = (long long)tile * TZ + zz + (long long)t * A.plane, estride = (long long)A.plane * TPP;
-    C* xs = s_x + tb * (N * TZ);
+    C* xs = s_x + grp * Cfg::XELEMS + tb * (N * TZ);
     const bool start = s < A.nsteps, keep = s <= A.dens.keep || s == A.nsteps;
     C* Fb = static_cast<C*>(A.F[b]); C* Hb = static_cast<C*>(A.H[b]);
+    if (grp == 1) {                                            // H = Dx'[e4 q_s], as soon as group 0 has formed e4 q_s
+        if (start) {
+            asm volatile("bar.sync 3, %0;" ::"n"(2 * NT) : "memory");
+            C v[EPT];
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
+            diffuse<T, N, EPT, NT, typename Cfg::LS, typename Cfg::LC, 2>(v, t, zz, false, s_tw, s_tab + N, xs, xs);
+            if (active) {
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) stcg(Hb + base0 + r * estride, v[r]);
+            }
+        }
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+        return;
+    }
     C* qs = static_cast<C*>(A.q[b]) + (long long)slice_slot(s, A.dens.keep) * A.M;
     const C* e4p = static_cast<const C*>(A.e4[sp_prev]); const C* e4n = static_cast<const C*>(A.e4[sp_now]);
 
@@ -243,17 +262,20 @@ __global__ void __launch_bounds__(128) tline_kernel(const TlineArgs A) {
             s_stash[r * NT + tid] = hb;
             v[r] = cmul(hb, e, cw);
         }
+        if constexpr (Cfg::SPLIT) asm volatile("bar.arrive 3, %0;" ::"n"(2 * NT) : "memory");      // e4 q_s is in shared memory: group 1 takes the half branch
         diffuse<T, N, EPT, NT, typename Cfg::LS, typename Cfg::LC>(v, t, zz, false, s_tw, s_tab, xs, s_x);
         if (active) {
 #pragma unroll
             for (int r = 0; r < EPT; ++r) stcg(Fb + base0 + r * estride, v[r]);
         }
+        if constexpr (!Cfg::SPLIT) {
 #pragma unroll
-        for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
-        diffuse<T, N, EPT, NT, typename Cfg::LS, typename Cfg::LC>(v, t, zz, false, s_tw, s_tab + N, xs, s_x);
-        if (active) {
+            for (int r = 0; r < EPT; ++r) v[r] = s_stash[r * NT + tid];
+            diffuse<T, N, EPT, NT, typename Cfg::LS, typename Cfg::LC>(v, t, zz, false, s_tw, s_tab + N, xs, s_x);
+            if (active) {
 #pragma unroll
-            for (int r = 0; r < EPT; ++r) stcg(Hb + base0 + r * estride, v[r]);
+                for (int r = 0; r < EPT; ++r) stcg(Hb + base0 + r * estride, v[r]);
+            }
         }
     }
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
