@@ -69,10 +69,11 @@ def test_config1_fp32(B, oracle):
     assert np.max(np.abs(pa.cpu().numpy() - oa)) < 2e-4 * np.max(np.abs(oa))
 
 
-@pytest.mark.parametrize("grid", [(8, 16, 32), (32, 8, 16), (16, 64, 8), (64, 32, 16)])
+@pytest.mark.parametrize("grid", [(8, 16, 32), (32, 8, 16), (16, 64, 8), (64, 32, 16), (8, 32, 32), (64, 16, 16), (16, 64, 64), (1, 32, 32)])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_ragged_diblock_complex_fields(B, oracle, grid, precision):
-    """Anisotropic grids: every pencil length 8..64 appears along every dimension; complex (CL-like) fields."""
+    """Anisotropic grids: every pencil length 8..64 appears along every dimension; complex (CL-like) fields.  The last four
+    have square yz-planes (the fused plane kernel) under an x dimension of a different length."""
     cfg = inputs.small_diblock(grid=grid, cell=(3.0, 4.0, 5.0), Ns=10, fA=0.4)
     g, o = _pair(B, oracle, cfg, precision=precision)
     if precision == "f64":
