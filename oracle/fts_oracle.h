@@ -19,8 +19,9 @@
  * dense matrix exponential, 4th-order convergence, mean_x q_j q+_{Ns-j} = Q, Debye response,
  * homogeneous saddles (diblock H, Edwards H/mu/Pi), Philox known-answer vectors; the SCFT multipliers and the
  * Eq. 10-11 (scheme 1) update, both models, to the backward-Euler / IMEX step of the linearised dynamics and to
- * exactly filtered noise at the saddle.  The Pi operator is "parity unpinned" beyond
- * a finite-difference dln Q/dV check and its mean-field value (derived, not printed in the paper).
+ * exactly filtered noise at the saddle.  The Pi operator (derived, reading A-14: the paper prints no formula) is pinned by
+ * its mean-field values and by finite-difference d ln Q/dV of its K term on both branches: one species, and the diblock
+ * with complex fields and unequal blocks (q+ != q), where the pin also rejects q_{Ns-j} or q+_j in place of q+_{Ns-j}.
  */
 #ifndef FTS_ORACLE_H
 #define FTS_ORACLE_H

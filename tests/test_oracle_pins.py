@@ -383,7 +383,7 @@ def test_edwards_H_at_the_homogeneous_saddle(oracle):
 
 
 def test_pressure_kernel_matches_volume_derivative_of_lnQ(oracle):
-    """-(2/3V) K = d ln Q / dV at fixed lattice fields (reading A-14; the only pin Pi has: 'parity unpinned')."""
+    """-(2/3V) K = d ln Q / dV at fixed lattice fields (reading A-14), one species: q+ = q.  The diblock branch has its own pin below."""
     cfg = inputs.config1(grid=(8, 8, 8), Ns=64)
     V = float(np.prod(cfg.cell))
 
@@ -399,6 +399,57 @@ def test_pressure_kernel_matches_volume_derivative_of_lnQ(oracle):
     _, o = lnQ(1.0)
     _, _, Pi = o.operators()                     # model 0: Pi = -(2/3) K
     assert abs(Pi / V - fd) < 5e-3 * abs(fd)
+
+
+def test_diblock_pressure_matches_volume_derivative_of_lnQ(oracle):
+    """The diblock branch Pi = C - (2C/3) K (reading A-14) with complex fields and unequal blocks, where q+ is NOT q: the
+    K term must still be the volume derivative of ln Q at fixed lattice fields, (Pi - C)/(C V) = -(2/3V) K = d ln Q / dV.
+    The pin tells q+_{Ns-j} from q_{Ns-j} (and from q+_j): K rebuilt from the oracle's own slices with either slip misses the
+    finite difference by far more than the tolerance."""
+    def case(Ns):
+        cfg = inputs.small_diblock(grid=(8, 8, 8), cell=(3.0, 3.5, 4.0), Ns=Ns, fA=0.25, complex_fields=True)
+        V, Cc = float(np.prod(cfg.cell)), cfg.C
+
+        def solve(scale):
+            cell = tuple(L * scale ** (1 / 3) for L in cfg.cell)
+            o = oracle.Oracle(cfg.grid, cell, cfg.Ns, "diblock", fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=Cc)
+            o.set_fields(cfg.f0, cfg.f1)
+            o.propagate()
+            return np.log(o.density_operators()[0]), o
+
+        d = 1e-4
+        fd = (solve(1 + d)[0] - solve(1 - d)[0]) / (2 * d * V)
+        _, o = solve(1.0)
+        _, _, Pi = o.operators()
+        return cfg, V, o, fd, (Pi - Cc) / (Cc * V)
+
+    # K is the derivative of the contour-continuous ln Q; the lattice ln Q converges to it with the contour step
+    # (measured: relative gap 4.0e-2, 5.9e-3, 6.6e-4, 5.7e-5 at Ns = 16, 32, 64, 128)
+    _, _, _, fd32, got32 = case(32)
+    cfg, V, o, fd, got = case(64)
+    assert abs(fd.imag) > 1e-3 * abs(fd.real) > 0            # genuinely complex: a conjugation slip would show
+    assert abs(got - fd) < 1e-3 * abs(fd), (got, fd)
+    assert abs(got - fd) / abs(fd) < 0.2 * abs(got32 - fd32) / abs(fd32)
+    # discriminating power: the same contour sum with q_{Ns-j} or q+_j in place of q+_{Ns-j}
+    Ns, jA = cfg.Ns, int(round(cfg.fA * cfg.Ns))
+    k = [2 * np.pi * np.fft.fftfreq(n, L / n) for n, L in zip(cfg.grid, cfg.cell)]
+    k2 = k[0][:, None, None] ** 2 + k[1][None, :, None] ** 2 + k[2][None, None, :] ** 2
+    simpson = lambda n: np.array([1.0] + [4.0 if i % 2 else 2.0 for i in range(1, n)] + [1.0]) / 3.0
+    c = np.zeros(Ns + 1); c[:jA + 1] += simpson(jA); c[jA:] += simpson(Ns - jA)
+    Q = o.density_operators()[0]
+
+    def K_of(partner):
+        tot = 0.0
+        for j in range(Ns + 1):
+            lap = np.fft.ifftn(-k2 * np.fft.fftn(o.get_slice(0, j)))
+            tot += c[j] * np.mean(partner(j) * lap)
+        return tot / (Ns * Q)
+
+    right = -(2.0 / (3.0 * V)) * K_of(lambda j: o.get_slice(1, Ns - j))
+    assert abs(right - fd) < 1e-3 * abs(fd)
+    for slip in (lambda j: o.get_slice(0, Ns - j), lambda j: o.get_slice(1, j)):
+        wrong = -(2.0 / (3.0 * V)) * K_of(slip)
+        assert abs(wrong - fd) > 2e-2 * abs(fd)
 
 
 # ------------------------------------------------------------------ Philox / noise --------------
