@@ -158,6 +158,35 @@ fts_status fts_debug_philox(uint64_t seed, uint64_t step, uint32_t field_id, uin
 fts_status fts_debug_fma_peak(int precision, int iters, void* scratch_dev, size_t scratch_bytes, double* fma_count, void* stream);
 uint64_t fts_launch_count(void);
 
+/* Mean of a complex field without any caller-provided or library-allocated scratch: mean_dev[0..1] = (re, im) of
+ * (1/npoints) sum_x field[x], accumulated in fp64.  With field = the last contour slice q(x,1) this is Q of PAPER.md:65
+ * Eq. 4, computed with the same fixed-order two-stage sum as fts_propagate (bit-identical to the Q it leaves behind).
+ *
+ * Why it exists: everything else in this header works inside the workspace handed to fts_create.  A caller may have no
+ * such memory to give and no way to get any - an observer inside another program's run that receives slice pointers
+ * but owns no context while the host program has already split all of HBM among its own buffers; code on a path where
+ * marches are in flight on other streams and the device-wide synchronisation cudaMalloc / cudaFree can cause is not
+ * acceptable; a process whose allocator must not see raw runtime allocations next to its pool.  For those the per-CTA
+ * partial sums live in a fixed array inside the library's device image (9472 bytes on every GPU that loads libfts.so,
+ * held until the process exits).  This call never calls cudaMalloc, cudaFree or any allocating routine.
+ *
+ * Arguments: field_dev - DEVICE, npoints interleaved (re, im) pairs of the given precision, read only; mean_dev - DEVICE,
+ * two doubles, written on `stream`; both stay the caller's.  errbuf (HOST, may be NULL) receives a NUL-terminated
+ * message of at most errbuf_len bytes when the status is not FTS_OK.  Asynchronous: nothing is synchronised.
+ * Limit: npoints <= FTS_MEAN_NOALLOC_MAX_POINTS (256^3, the largest grid of this library); above it FTS_EUNSUPPORTED with
+ * a message, nothing launched.  FTS_EINVAL: NULL field_dev / mean_dev, npoints = 0, unknown precision.  FTS_ECUDA: the
+ * address look-up or a launch failed.
+ * First call per device: looks up the array's device address once, with the current device (this can initialise the
+ * CUDA context and load the device code) - make it at start-up, with the intended device current, before any stream
+ * capture on that device.  Later calls only enqueue two small kernels on the current device.
+ * Shared state: every call on a device uses the same array.  Nothing in it needs zeroing (each call overwrites exactly
+ * the partials it then reads), but calls that can overlap on one GPU - different streams, or host threads using
+ * different streams - race on it and return wrong means.  Keep them on one stream or order them with events.
+ * Not counted by fts_launch_count. */
+#define FTS_MEAN_NOALLOC_MAX_POINTS 16777216
+fts_status fts_mean_noalloc(const void* field_dev, size_t npoints, fts_precision prec, double* mean_dev, void* stream,
+                            char* errbuf, size_t errbuf_len);
+
 const char* fts_last_error(const fts_ctx* ctx);
 const char* fts_version(void);
 

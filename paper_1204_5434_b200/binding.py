@@ -16,7 +16,7 @@ STATUS = {0: "FTS_OK", 1: "FTS_EINVAL", 2: "FTS_ESTATE", 3: "FTS_EWORKSPACE", 4:
 MODELS = {"external": 0, "edwards": 1, "diblock": 2}
 EXPORTS = ["fts_workspace_bytes", "fts_create", "fts_destroy", "fts_set_fields", "fts_get_fields", "fts_propagate",
            "fts_propagate_steps", "fts_set_blocks", "fts_density_operators", "fts_get_slice", "fts_scft_step", "fts_cl_step",
-           "fts_operators", "fts_set_option", "fts_debug_normals", "fts_debug_philox", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
+           "fts_operators", "fts_set_option", "fts_mean_noalloc", "fts_debug_normals", "fts_debug_philox", "fts_debug_fma_peak", "fts_launch_count", "fts_last_error", "fts_version"]
 
 
 class FtsParams(C.Structure):
@@ -59,6 +59,7 @@ def lib():
         L.fts_debug_normals.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
         L.fts_debug_philox.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64, C.c_size_t, vp, vp]
         L.fts_debug_fma_peak.argtypes = [C.c_int, C.c_int, vp, C.c_size_t, dp, vp]
+        L.fts_mean_noalloc.argtypes = [vp, C.c_size_t, C.c_int, vp, vp, C.c_char_p, C.c_size_t]
         L.fts_launch_count.restype = C.c_uint64
         L.fts_last_error.argtypes = [vp]
         L.fts_last_error.restype = C.c_char_p
@@ -181,6 +182,27 @@ class Fts:
         H, mu, Pi = (C.c_double * 2)(), (C.c_double * 2)(), (C.c_double * 2)()
         self._chk(lib().fts_operators(self.h, H, mu, Pi if want_pi else None, _stream()), "fts_operators")
         return complex(H[0], H[1]), complex(mu[0], mu[1]), complex(Pi[0], Pi[1])
+
+
+MEAN_NOALLOC_MAX_POINTS = 1 << 24      # FTS_MEAN_NOALLOC_MAX_POINTS of include/fts.h
+
+
+def mean_noalloc(field, out, npoints=None):
+    """fts_mean_noalloc: enqueue mean(field) -> out (2 float64 on the device: re, im) on the current stream of field's
+    device.  For callers that own no workspace and may not allocate (see include/fts.h): the library's reduction scratch
+    is a fixed array inside libfts.so, so neither this wrapper nor the library allocates anything - `out` is the
+    caller's, which is why it is not optional.  Calls that may overlap on one GPU (different streams) race on that array.
+    The first call on a device does a one-time address look-up: make it before any stream capture.  npoints overrides
+    field.numel() (tests of the size limit).  Returns `out`; nothing is synchronised."""
+    assert field.is_cuda and field.is_contiguous() and field.dtype in (torch.complex128, torch.complex64)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 2 and out.is_contiguous() and out.device == field.device
+    n = field.numel() if npoints is None else int(npoints)
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(field.device):
+        rc = lib().fts_mean_noalloc(_p(field), n, 0 if field.dtype == torch.complex128 else 1, _p(out), _stream(), err, len(err))
+    if rc:
+        raise FtsError("fts_mean_noalloc", rc, err.value.decode())
+    return out
 
 
 def debug_normals(seed, step, field_id, site0, n, device="cuda:0"):
