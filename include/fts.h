@@ -134,7 +134,7 @@ fts_status fts_operators(fts_ctx* ctx, double H[2], double mu[2], double Pi[2], 
  *   "tz"          modes 1-2: pencils per strided tile, 8 or 16 (0 = default)
  *   "graph"       mode 1: replay the march's launches as one CUDA graph, captured once per context (default 1)
  *   "tline"       mode 1: straight-line kernel for the x pass of a step when Nx <= 64 (default 1)
- *   "plane"       mode 1: fuse the y and z passes of a step into one kernel per yz-plane when Ny = Nz = 16 or 32 (default 1)
+ *   "plane"       mode 1: fuse the y and z passes of a step into one kernel per yz-plane when Ny = Nz = 16, 32 or 64 (default 1)
  *   "real_fields" 1: the caller declares that W+ and W- are real (SCFT; diblock only).  q and q+ are then
  *                 real and are marched together as ONE complex propagator z = q + i q+ (half the transforms and slices);
  *                 results agree with the general path to rounding; phi and slices are returned with zero imaginary part.

@@ -519,7 +519,7 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
             const int gb = gbase_of();
             const C* partner = static_cast<const C*>(A.q[two ? 1 - b : 0]) + (size_t)(A.Ns - s) * N * N * N + gb;
             for (int pass = 0; pass < 2; ++pass) {                      // sums of species A, then B (both only at the block junction)
-                const T w1 = pass == 0 ? wA : wB, w2 = pass == 0 ? wA2 : wB2;
+                const T w1 = pass == 0 ? wA : wB;
                 if (cw ? pass == 1 : w1 == (T)0) continue;
                 C* acc = static_cast<C*>(A.dens.acc[b][cw ? 0 : pass]) + gb;
 #pragma unroll 1
@@ -544,7 +544,6 @@ __global__ void __launch_bounds__(M2_LAUNCH, (sizeof(T) == 8 ? 2 : 4)) march2_ke
                         }
                     }
                 }
-                (void)w2;
             }
         };
         // L2 prefetch of what accumulate_density will read (issued when the item starts, a transform ahead of its use)

@@ -7,7 +7,7 @@
 // -> inverse, which is the operator exp(ds * d^2/dx_d^2) of PAPER.md:124-127 (Eq. 12) along one dimension;
 // the 3-D operator is the product of the three 1-D ones because exp(-k^2 ds) factorises.
 //
-// Layout facts the kernels rely on (checked on the host by tests/test_host_pencil.py):
+// Layout facts the kernels rely on (checked on the host by tests/host_pencil_test.cpp):
 //   * natural layout:  register r of thread t holds point  n = t + TPP*r
 //   * spectral layout: register r of thread t holds mode   k = t + TPP*r   (same map: tables need no permutation)
 //
