@@ -90,7 +90,9 @@ def workspace_bytes(grid, Ns, params, precision="f64"):
 
 
 class Fts:
-    """One simulation context on the current CUDA device.  Methods mirror the C calls one to one."""
+    """One simulation context on `device`.  Methods mirror the C calls one to one; each makes the context's device current
+    for the duration of the call (the library launches on the current device), so a context on cuda:1 can be driven
+    while cuda:0 is the process's current device.  The stream is the current stream OF THAT DEVICE."""
 
     def __init__(self, grid, cell, Ns, model, precision="f64", device="cuda:0", options=None, **kw):
         self.grid = tuple(int(v) for v in grid)
@@ -125,7 +127,8 @@ class Fts:
 
     def close(self):
         if getattr(self, "h", None) and _lib is not None:
-            _lib.fts_destroy(self.h)
+            with torch.cuda.device(self.device):
+                _lib.fts_destroy(self.h)
         self.h = None
 
     def __del__(self):
@@ -144,43 +147,51 @@ class Fts:
     def set_fields(self, f0, f1=None):
         assert f0.is_cuda and f0.dtype == self.cdtype and f0.is_contiguous() and tuple(f0.shape) == self.grid
         assert f1 is None or (f1.is_cuda and f1.dtype == self.cdtype and f1.is_contiguous())
-        self._chk(lib().fts_set_fields(self.h, _p(f0), _p(f1), _stream()), "fts_set_fields")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_set_fields(self.h, _p(f0), _p(f1), _stream()), "fts_set_fields")
 
     def get_fields(self):
         a = self._new()
         b = self._new() if self.model == 2 else None
-        self._chk(lib().fts_get_fields(self.h, _p(a), _p(b), _stream()), "fts_get_fields")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_get_fields(self.h, _p(a), _p(b), _stream()), "fts_get_fields")
         return a, b
 
     def propagate(self, nsteps=None):
-        if nsteps is None:
-            self._chk(lib().fts_propagate(self.h, _stream()), "fts_propagate")
-        else:
-            self._chk(lib().fts_propagate_steps(self.h, int(nsteps), _stream()), "fts_propagate_steps")
+        with torch.cuda.device(self.device):
+            if nsteps is None:
+                self._chk(lib().fts_propagate(self.h, _stream()), "fts_propagate")
+            else:
+                self._chk(lib().fts_propagate_steps(self.h, int(nsteps), _stream()), "fts_propagate_steps")
 
     def density_operators(self, phiA=None, phiB=None):
         phiA = self._new() if phiA is None else phiA
         phiB = (self._new() if phiB is None else phiB) if self.model == 2 else None
         Q = (C.c_double * 2)()
-        self._chk(lib().fts_density_operators(self.h, _p(phiA), _p(phiB), Q, _stream()), "fts_density_operators")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_density_operators(self.h, _p(phiA), _p(phiB), Q, _stream()), "fts_density_operators")
         return complex(Q[0], Q[1]), phiA, phiB
 
     def get_slice(self, which, j, out=None):
         out = self._new() if out is None else out
-        self._chk(lib().fts_get_slice(self.h, int(which), int(j), _p(out), _stream()), "fts_get_slice")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_get_slice(self.h, int(which), int(j), _p(out), _stream()), "fts_get_slice")
         return out
 
     def scft_step(self, dt_plus, dt_minus, seidel=1):
         H, r = (C.c_double * 2)(), (C.c_double * 2)()
-        self._chk(lib().fts_scft_step(self.h, dt_plus, dt_minus, int(seidel), H, r, _stream()), "fts_scft_step")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_scft_step(self.h, dt_plus, dt_minus, int(seidel), H, r, _stream()), "fts_scft_step")
         return complex(H[0], H[1]), (r[0], r[1])
 
     def cl_step(self, dt, scheme, seed, step):
-        self._chk(lib().fts_cl_step(self.h, dt, int(scheme), int(seed), int(step), _stream()), "fts_cl_step")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_cl_step(self.h, dt, int(scheme), int(seed), int(step), _stream()), "fts_cl_step")
 
     def operators(self, want_pi=True):
         H, mu, Pi = (C.c_double * 2)(), (C.c_double * 2)(), (C.c_double * 2)()
-        self._chk(lib().fts_operators(self.h, H, mu, Pi if want_pi else None, _stream()), "fts_operators")
+        with torch.cuda.device(self.device):
+            self._chk(lib().fts_operators(self.h, H, mu, Pi if want_pi else None, _stream()), "fts_operators")
         return complex(H[0], H[1]), complex(mu[0], mu[1]), complex(Pi[0], Pi[1])
 
 
@@ -207,7 +218,8 @@ def mean_noalloc(field, out, npoints=None):
 
 def debug_normals(seed, step, field_id, site0, n, device="cuda:0"):
     out = torch.empty(n, dtype=torch.float64, device=device)
-    rc = lib().fts_debug_normals(int(seed), int(step), int(field_id), int(site0), int(n), _p(out), _stream())
+    with torch.cuda.device(out.device):
+        rc = lib().fts_debug_normals(int(seed), int(step), int(field_id), int(site0), int(n), _p(out), _stream())
     if rc:
         raise FtsError("fts_debug_normals", rc)
     return out
@@ -216,7 +228,8 @@ def debug_normals(seed, step, field_id, site0, n, device="cuda:0"):
 def debug_philox(seed, step, field_id, site0, n, device="cuda:0"):
     """(n, 4) int64 tensor holding the raw 32-bit Philox words of sites site0 .. site0 + n - 1."""
     out = torch.empty((n, 4), dtype=torch.int32, device=device)
-    rc = lib().fts_debug_philox(int(seed), int(step), int(field_id), int(site0), int(n), _p(out), _stream())
+    with torch.cuda.device(out.device):
+        rc = lib().fts_debug_philox(int(seed), int(step), int(field_id), int(site0), int(n), _p(out), _stream())
     if rc:
         raise FtsError("fts_debug_philox", rc)
     return out.to(torch.int64) & 0xFFFFFFFF
@@ -229,8 +242,9 @@ def launch_count():
 def fma_peak_launch(precision, iters, scratch):
     """Enqueue the FMA-chain kernel on the current stream; returns the FMA count of that launch."""
     n = C.c_double()
-    rc = lib().fts_debug_fma_peak(0 if precision == "f64" else 1, int(iters), _p(scratch), scratch.numel() * scratch.element_size(),
-                                  C.byref(n), _stream())
+    with torch.cuda.device(scratch.device):
+        rc = lib().fts_debug_fma_peak(0 if precision == "f64" else 1, int(iters), _p(scratch), scratch.numel() * scratch.element_size(),
+                                      C.byref(n), _stream())
     if rc:
         raise FtsError("fts_debug_fma_peak", rc)
     return n.value
