@@ -329,18 +329,21 @@ def oracle_cfg5s(oracle):
     o.propagate()
     Q, pa, pb = o.density_operators()
     qN = o.get_slice(0, cfg.Ns)
+    ops = o.operators()                                # H, mu, Pi out of the same solve (Pi: 101 Laplacians, ~40 s)
     o.cl_step(cfg.dt, 0, CL_SEED, 0)
     wp, wm = o.get_fields()
     del o
-    return cfg, Q, pa, pb, qN, wp, wm
+    return cfg, Q, pa, pb, qN, wp, wm, ops
 
 
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_config5s_full_oracle_solve_and_cl_step(B, oracle_cfg5s, precision):
-    """SURVEY 8(d), config 5s in the launch configuration bench.py times (TMA march, default store): Q to 1e-11 (2e-4 in
-    complex64), phi_A, phi_B and q(r,1) element-wise to 1e-9 (2e-4), and the fields after one fts_cl_step with identical Philox
-    noise to 1e-9 (2e-4), all against the oracle's full 200-step solve."""
-    cfg, Qo, oa, ob, qN, wpo, wmo = oracle_cfg5s
+    """SURVEY 8(d), config 5s through the TMA march in BOTH slice stores - the library default (meet-in-the-middle, densities
+    fused into the march) and the full store bench.py times by default (store_both = 1, densities by density_store_kernel):
+    Q to 1e-11 (2e-4 in complex64), phi_A, phi_B and q(r,1) element-wise to 1e-9 (2e-4), the fields after one fts_cl_step with
+    identical Philox noise to 1e-9 (2e-4), and - N2 at scale, full store - H, mu and Pi over the 2 x 101 stored slices of 128^3,
+    all against the oracle's full 200-step solve."""
+    cfg, Qo, oa, ob, qN, wpo, wmo, ops_o = oracle_cfg5s
     dt = torch.complex128 if precision == "f64" else torch.complex64
     tq, tp = (1e-11, 1e-9) if precision == "f64" else (2e-4, 2e-4)
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
@@ -352,6 +355,20 @@ def test_config5s_full_oracle_solve_and_cl_step(B, oracle_cfg5s, precision):
     assert np.max(np.abs(g.get_slice(0, cfg.Ns).cpu().numpy() - qN)) <= tp * max(1.0, np.max(np.abs(qN)))
     g.cl_step(cfg.dt, 0, CL_SEED, 0)
     wp, wm = g.get_fields()
+    assert np.max(np.abs(wp.cpu().numpy() - wpo)) <= tp * max(1.0, np.max(np.abs(wpo)))
+    assert np.max(np.abs(wm.cpu().numpy() - wmo)) <= tp * max(1.0, np.max(np.abs(wmo)))
+    g.close(); del g
+    f = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=1, **_kw(cfg))      # bench.py --store full
+    f.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))
+    f.propagate()
+    Qf, fa, fb = f.density_operators()
+    assert abs(Qf - Qo) <= tq * abs(Qo), (Qf, Qo)
+    assert np.max(np.abs(fa.cpu().numpy() - oa)) <= tp and np.max(np.abs(fb.cpu().numpy() - ob)) <= tp
+    for k, (x, y) in enumerate(zip(f.operators(), ops_o)):      # H/(CV), mu = ln C - ln Q, Pi (reading A-14)
+        tol = 1e-9 if precision == "f64" else (2e-4 if k < 2 else 5e-3)      # complex64 Pi: -k^2 amplifies the rounding of 101 slices
+        assert abs(x - y) <= tol * max(1.0, abs(y)), (k, x, y)
+    f.cl_step(cfg.dt, 0, CL_SEED, 0)
+    wp, wm = f.get_fields()
     assert np.max(np.abs(wp.cpu().numpy() - wpo)) <= tp * max(1.0, np.max(np.abs(wpo)))
     assert np.max(np.abs(wm.cpu().numpy() - wmo)) <= tp * max(1.0, np.max(np.abs(wmo)))
 
@@ -404,10 +421,13 @@ def test_config5_truncated_march_and_invariants(B, oracle_cfg5_first8, precision
 # "developed" fields (inputs.developed: nothing the CUDA path produced is ever fed to the oracle); and properties that
 # hold at any size after a long GPU run (the oracle is too slow for 200-1000 iterations)
 # ------------------------------------------------------------------------------------------------
-def _developed_solve_parity(B, oracle, cfg, precision="f64", tolQ=1e-11, tolphi=1e-9, operators=False):
+def _developed_solve_parity(B, oracle, cfg, precision="f64", tolQ=1e-11, tolphi=1e-9, operators=False, real_fields=False):
     f0, f1 = inputs.developed(cfg)
     dt = torch.complex128 if precision == "f64" else torch.complex64
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, store_both=1 if operators else 0, **_kw(cfg))
+    if real_fields:                                    # the real parts of the developed fields, marched packed (z = q + i q+)
+        f0, f1 = np.ascontiguousarray(f0.real).astype(np.complex128), np.ascontiguousarray(f1.real).astype(np.complex128)
+        g.set_option("real_fields", 1)
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
     g.set_fields(_dev(f0, dt), None if f1 is None else _dev(f1, dt))
     o.set_fields(f0, f1)
@@ -442,10 +462,17 @@ def test_config2_scft_full_size(B, oracle):
     GPU (residual falls, invariants hold); one solve at developed fields against the oracle."""
     cfg = inputs.config2()
     g, o = _pair(B, oracle, cfg)
+    gr, _ = _pair(B, oracle, cfg, store_both=0)         # as bench.py runs SCFT workloads: real_fields = 1, q and q+ packed, Ns = 100, jA = 30
+    gr.set_option("real_fields", 1)
     for it in range(4):
         Hg, rg = g.scft_step(*cfg.dt_scft, 1)
+        Hr, rr = gr.scft_step(*cfg.dt_scft, 1)
         Ho, ro = o.scft_step(*cfg.dt_scft, 1)
         assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9, it
+        assert abs(Hr - Ho) < 1e-10 and abs(rr[0] - ro[0]) < 1e-9 and abs(rr[1] - ro[1]) < 1e-9, it
+    for x, y in zip(gr.get_fields(), o.get_fields()):
+        assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+    _developed_solve_parity(B, oracle, cfg, real_fields=True)
     res = []
     for it in range(4, cfg.iters):
         H, r = g.scft_step(*cfg.dt_scft, 1)
@@ -463,11 +490,18 @@ def test_config3_scft_full_size(B, oracle, precision):
     cfg = inputs.config3()
     g, o = _pair(B, oracle, cfg, precision=precision)
     if precision == "f64":                             # one Seidel iteration side by side (2 x 400 RQM4 steps on the oracle, ~75 s)
+        gr, _ = _pair(B, oracle, cfg, store_both=0)     # ... and the same iteration as bench.py runs it: real_fields = 1 (packed march, Ns = 200, jA = 70)
+        gr.set_option("real_fields", 1)
         Hg, rg = g.scft_step(*cfg.dt_scft, 1)
+        Hr, rr = gr.scft_step(*cfg.dt_scft, 1)
         Ho, ro = o.scft_step(*cfg.dt_scft, 1)
         assert abs(Hg - Ho) < 1e-10 and abs(rg[0] - ro[0]) < 1e-9 and abs(rg[1] - ro[1]) < 1e-9
+        assert abs(Hr - Ho) < 1e-10 and abs(rr[0] - ro[0]) < 1e-9 and abs(rr[1] - ro[1]) < 1e-9
         for x, y in zip(g.get_fields(), o.get_fields()):
             assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+        for x, y in zip(gr.get_fields(), o.get_fields()):
+            assert np.max(np.abs(x.cpu().numpy() - y)) < 1e-9
+        gr.close(); del gr
     del o
     for it in range(30):
         H, r = g.scft_step(*cfg.dt_scft, 1)
@@ -475,20 +509,24 @@ def test_config3_scft_full_size(B, oracle, precision):
     _invariants(g, cfg, 1e-11 if precision == "f64" else 2e-4)
     if precision == "f64":
         _developed_solve_parity(B, oracle, cfg)
+        _developed_solve_parity(B, oracle, cfg, real_fields=True)      # the packed march at developed (real) fields, ~40 s of oracle
     else:
         _developed_solve_parity(B, oracle, cfg, precision="f32", tolQ=2e-4, tolphi=2e-4)
 
 
 def test_config4_edwards_cl_full_size(B, oracle):
-    """64^3 Edwards solution, B = 1, C = 10, dt = 0.01: 2 CL steps side by side (identical Philox noise); 100 more steps on
-    the GPU (invariants); one solve plus the operators H, mu, Pi at developed fields against the oracle."""
+    """64^3 Edwards solution, B = 1, C = 10, dt = 0.01: north_star's criterion at the config's own size - 10 CL steps side by
+    side with identical Philox noise, fields within 1e-8 (~95 s of oracle); 100 more steps on the GPU (invariants); one solve
+    plus the operators H, mu, Pi at developed fields against the oracle."""
     cfg = inputs.config4()
     g, o = _pair(B, oracle, cfg)
-    for step in range(2):
+    for step in range(10):
         g.cl_step(cfg.dt, 0, 4242, step); o.cl_step(cfg.dt, 0, 4242, step)
+        if step == 1:
+            assert np.max(np.abs(g.get_fields()[0].cpu().numpy() - o.get_fields()[0])) < 1e-9
     a, _ = g.get_fields(); oa, _ = o.get_fields()
-    assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-9
-    for step in range(2, 102):
+    assert np.max(np.abs(a.cpu().numpy() - oa)) < 1e-8
+    for step in range(10, 110):
         g.cl_step(cfg.dt, 0, 4242, step)
     _invariants(g, cfg, 1e-11)
     _developed_solve_parity(B, oracle, cfg, operators=True)
@@ -781,3 +819,36 @@ def test_streams_contexts_and_lifecycle(B, oracle):
         t.propagate(4); t.propagate()
         assert t.density_operators()[0] == Q0, rep
         t.close()
+
+
+def test_state_is_invalidated_by_set_option_and_set_blocks(B, oracle):
+    """After fts_cl_step, fts_operators reports the operators of the step's entry fields out of what the step left behind.  A
+    change of plan (fts_set_option) or of the chain architecture (fts_set_blocks) invalidates that: FTS_ESTATE until the next
+    solve, not numbers of the old chain.  Switching real_fields off ends the 'fields are not real' condition: the general path
+    then works on the same complex fields without an fts_set_fields in between; a failed fts_set_option leaves the context usable."""
+    cfg = inputs.small_diblock(grid=(16, 16, 16), Ns=12, fA=1.0 / 3.0)
+    for change in (lambda g: g.set_option("lag", 1), lambda g: g.set_blocks([0, 1, 0], [2, 6, 4])):
+        g, o = _pair(B, oracle, cfg)
+        g.cl_step(0.01, 0, 5, 0)
+        g.operators()                                   # allowed: the step's own solve
+        g.cl_step(0.01, 0, 5, 1)
+        change(g)
+        with pytest.raises(B.FtsError) as e:
+            g.operators()
+        assert e.value.status == 2                      # FTS_ESTATE
+        g.propagate()
+        g.operators()
+    g, o = _pair(B, oracle, cfg)                        # complex fields
+    g.set_option("real_fields", 1)
+    g.propagate()
+    with pytest.raises(B.FtsError) as e:
+        g.density_operators()
+    assert e.value.status == 1                          # FTS_EINVAL: the declaration was wrong
+    g.set_option("real_fields", 0)                      # ... and is withdrawn: no fts_set_fields needed
+    _cmp_solve(g, o, 1e-11, 1e-9, True)
+    with pytest.raises(B.FtsError) as e:
+        g.set_option("march", 3)                        # TMA march on a 16^3 grid: refused, nothing changed
+    assert e.value.status == 6
+    g.propagate()
+    Qg, _, _ = g.density_operators(); Qo, _, _ = o.density_operators()
+    assert abs(Qg - Qo) <= 1e-11 * abs(Qo)
