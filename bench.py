@@ -206,6 +206,89 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+TRAFFIC_SOURCES = ("fts_march2.cuh", "fts_pencil.h")      # the files that define the kernel profiles/traffic.json was captured from
+
+
+def march_source_sha():
+    """sha256 over the march kernel's source files (there is no .git on the GPU box, so the stamp is a content hash)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in TRAFFIC_SOURCES:
+        h.update(open(os.path.join(ROOT, "paper_1204_5434_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def executed_rqm4_per_propagate(cfg, opts):
+    """RQM4 steps one fts_propagate EXECUTES: q and q+ share one packed march under real_fields (the roofline
+    counts executed work; the headline metric keeps counting the method's two propagators)."""
+    nprop = 2 if cfg.model == "diblock" else 1
+    return (1 if opts.get("real_fields") else nprop) * cfg.Ns
+
+
+def fma_peak_tflops(B, prec, dev):
+    """Vector-FMA peak of this GPU in `prec`, register-resident chains timed with CUDA events; best of 3."""
+    import torch
+    scratch = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
+    B.fma_peak_launch(prec, 512, scratch)
+    best = 0.0
+    for _ in range(3):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        nf = B.fma_peak_launch(prec, 8192, scratch)
+        b.record()
+        torch.cuda.synchronize()
+        best = max(best, 2.0 * nf / (a.elapsed_time(b) * 1e-3) / 1e12)
+    return best
+
+
+def roofline_core(M, E, rq_exec, ms_march, peak_tflops, hbm_gbs):
+    """F_alg = 30 M log2 M flop and B_alg = 3 E M bytes per executed RQM4 step of one propagator."""
+    f_alg, b_alg = 30.0 * M * math.log2(M), 3.0 * E * M
+    t_fp, t_hbm = f_alg / (peak_tflops * 1e12), b_alg / (hbm_gbs * 1e9)
+    t_step = ms_march * 1e-3 / rq_exec
+    if t_fp >= t_hbm:
+        core = {"bound": "alu", "achieved": f_alg / t_step / 1e12, "peak": peak_tflops, "unit": "TFLOP/s", "frac": t_fp / t_step}
+    else:
+        core = {"bound": "hbm", "achieved": b_alg / t_step / 1e9, "peak": hbm_gbs, "unit": "GB/s", "frac": t_hbm / t_step}
+    return core, f_alg, b_alg, t_hbm / t_step
+
+
+def also_measure(B, workload, prec, store, steps, warmup, dev, flush, peak_tflops, hbm_gbs, seed):
+    """One more shape of the north_star target, measured in the same run with the same events: the whole step
+    (value, ms_per_step) and fts_propagate alone (march_ms, roofline fraction)."""
+    import torch
+    cfg, kind = make_workload(workload)
+    cdt = torch.complex128 if prec == "f64" else torch.complex64
+    M, E = int(np.prod(cfg.grid)), (16 if prec == "f64" else 8)
+    g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=prec, device=dev, fA=cfg.fA, chiN=cfg.chiN, B=cfg.B, Cc=cfg.C,
+              store_both=1 if store == "full" else 0)
+    g.set_fields(*[torch.from_numpy(np.ascontiguousarray(f)).to(cdt).to(dev) for f in (cfg.f0, cfg.f1) if f is not None])
+
+    def timed(fn, n, first):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for i in range(n):
+            flush.zero_()
+            ev[i][0].record()
+            fn(first + i)
+            ev[i][1].record()
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev)
+
+    for i in range(warmup):
+        g.cl_step(cfg.dt, 0, seed, i)
+    ms = timed(lambda i: g.cl_step(cfg.dt, 0, seed, i), steps, warmup)
+    g.propagate()
+    ms_march = timed(lambda i: g.propagate(), steps, 0) / steps
+    rq = executed_rqm4_per_propagate(cfg, {})
+    core, _, _, _ = roofline_core(M, E, rq, ms_march, peak_tflops, hbm_gbs)
+    out = {"workload": cfg.name, "precision": prec, "slice_store": store, "value": M * rqm4_steps_per_step(cfg, kind) * steps / (ms * 1e-3), "unit": UNIT,
+           "ms_per_step": ms / steps, "march_ms": ms_march, "workspace_GB": round(g.workspace.numel() / 1e9, 2), "roofline": core}
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+    return out
+
+
 def max_over_ranks(values, device, world):
     """Device times of one replica per rank -> the slowest rank's (the job is as slow as its slowest replica).
     Replicas share nothing on the data path, so this is the only collective of the bench."""
@@ -313,16 +396,7 @@ def run_gpu(args):
     march_launches = (B.launch_count() - l0) // args.steps
 
     # vector-FMA peak of this GPU, measured with the same events
-    scratch = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
-    B.fma_peak_launch(prec, 512, scratch)
-    best = 0.0
-    for _ in range(3):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        nf = B.fma_peak_launch(prec, 8192, scratch)
-        b.record()
-        torch.cuda.synchronize()
-        best = max(best, 2.0 * nf / (a.elapsed_time(b) * 1e-3) / 1e12)
+    best = fma_peak_tflops(B, prec, dev)
 
     ms, ms_e2e, ms_march = max_over_ranks([ms, ms_e2e, ms_march], dev, world)
     if rank != 0:
@@ -333,27 +407,30 @@ def run_gpu(args):
     units = M * rqm4_steps_per_step(cfg, kind)                # per step per GPU
     value = world * units * args.steps / (ms * 1e-3)
     pk, pk_kind = peaks()
-    rq = nprop * cfg.Ns                                        # RQM4 steps in one fts_propagate
-    f_alg, b_alg = 30.0 * M * math.log2(M), 3.0 * E * M        # per RQM4 step of one propagator
-    t_fp, t_hbm = f_alg / (best * 1e12), b_alg / (pk["hbm_gbs"] * 1e9)
+    rq = executed_rqm4_per_propagate(cfg, opts)                # RQM4 steps one fts_propagate executes (packed march: Ns, not 2 Ns)
+    roof, f_alg, b_alg, hbm_frac = roofline_core(M, E, rq, ms_march, best, pk["hbm_gbs"])
     t_step = ms_march * 1e-3 / rq
+    if roof["bound"] == "alu":
+        roof["peak_kind"] = f"vector {prec} FMA chains measured in this run (nominal {FP64_NOMINAL_TFLOPS if prec == 'f64' else FP32_NOMINAL_TFLOPS:.1f})"
+    else:
+        roof["peak_kind"] = pk_kind
+    if opts.get("real_fields"):
+        roof["counts"] = ("executed work: q and q+ march packed as ONE complex propagator (real_fields), Ns RQM4 steps per solve; the headline metric counts "
+                          "the method's 2 Ns, so value / (M * achieved-rate) differs by that factor 2")
+        roof["frac_if_method_steps_counted"] = 2.0 * roof["frac"]
     pass_launches = max(1, march_launches - 3)                 # fts_propagate = boltzmann + march launch(es) + 2 reduction kernels; cubic grids: ONE persistent march launch
-    traffic, traffic_src = None, None
+    traffic, traffic_src, traffic_stale = None, None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         tj = json.load(open(tp))
-        traffic = tj.get(f"{args.workload}_{prec}")
-        traffic_src = {k: tj.get(k) for k in ("_note", "_commit", "_sm_mhz")}
-    if t_fp >= t_hbm:
-        roof = {"bound": "alu", "achieved": f_alg / t_step / 1e12, "peak": best, "unit": "TFLOP/s", "frac": t_fp / t_step,
-                "peak_kind": f"vector {prec} FMA chains measured in this run (nominal {FP64_NOMINAL_TFLOPS if prec == 'f64' else FP32_NOMINAL_TFLOPS:.1f})"}
-    else:
-        roof = {"bound": "hbm", "achieved": b_alg / t_step / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": t_hbm / t_step, "peak_kind": pk_kind}
-    roof.update({"traffic": traffic, "traffic_source": traffic_src, "kernel": "march2_kernel (128^3, 256^3) / march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve" + (")" if args.store == "full" else ", densities accumulated in the T items)"), "launches_per_march": pass_launches,
+        traffic = tj.get(f"{args.workload}_{prec}_{args.store}", tj.get(f"{args.workload}_{prec}") if args.store == "full" else None)
+        traffic_src = {k: tj.get(k) for k in ("_note", "_commit", "_sm_mhz", "_source_sha")}
+        traffic_stale = tj.get("_source_sha") != march_source_sha()      # the kernel's source changed since the ncu capture
+    roof.update({"traffic": traffic, "traffic_source": traffic_src, "traffic_stale": traffic_stale, "kernel": "march2_kernel (128^3, 256^3) / march_kernel (persistent: all T/Y1/Z/Y2 items of one propagator solve" + (")" if args.store == "full" else ", densities accumulated in the T items)"), "launches_per_march": pass_launches,
                  "avg_launch_us": ms_march * 1e3 / pass_launches, "alg_flops_per_launch": f_alg * rq / pass_launches,
                  "alg_bytes_per_launch": b_alg * rq / pass_launches, "march_ms": ms_march, "march_launches_all_kernels": march_launches,
                  "hbm_view": {"achieved_GBs_algorithmic": b_alg / t_step / 1e9, "peak_GBs": pk["hbm_gbs"], "peak_kind": pk_kind,
-                              "frac_of_floor": t_hbm / t_step}})
+                              "frac_of_floor": hbm_frac}})
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
            "config": config_dict(cfg, kind, prec, world, run_extras(args, kind)), "workspace_GB": round(g.workspace.numel() / 1e9, 2),
@@ -363,6 +440,21 @@ def run_gpu(args):
            "e2e": {"value": world * units * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": sum(h.numel() * h.element_size() for h in host),
                    "d2h_bytes_per_step": sum(b.numel() * b.element_size() for b in back[:1 if kind == 'propagate' else None])},
            "gpu_launches": launches, "roofline": roof}
+    if world == 1 and args.workload == "cfg5" and prec == "f64" and not args.opt and not args.no_also:
+        # the other shapes north_star names (128^3, fp32) and the library-default store, same run, same events
+        g.close()
+        del g, devf
+        torch.cuda.empty_cache()
+        best32 = fma_peak_tflops(B, "f32", dev)
+        also = {}
+        for wl, pr, st in (("cfg5", "f64", "mitm" if args.store == "full" else "full"), ("cfg5s", "f64", args.store), ("cfg5s", "f32", args.store), ("cfg5", "f32", args.store)):
+            try:
+                also[f"{wl}_{pr}_{st}"] = also_measure(B, wl, pr, st, args.steps, 3, dev, flush, best if pr == "f64" else best32, pk["hbm_gbs"], seed)
+                if os.path.exists(tp):                           # ncu DRAM bytes of that variant's march launch (same stamp as roofline.traffic)
+                    also[f"{wl}_{pr}_{st}"]["roofline"]["traffic"] = tj.get(f"{wl}_{pr}_{st}", tj.get(f"{wl}_{pr}") if st == "full" else None)
+            except Exception as e:                               # context: never lose the bench line over it
+                also[f"{wl}_{pr}_{st}"] = {"unavailable": repr(e)}
+        out["also"] = also
     if world == 1 and not args.no_cpu_baseline:
         v, dt, what = oracle_sample(cfg, 20.0)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what, "seconds": dt}
@@ -386,6 +478,7 @@ def main():
     ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="default workload only: skip the extra shapes (128^3, fp32, the other slice store) of the `also` block")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="fts_set_option (tuning experiments), e.g. --opt march=2")
     ap.add_argument("--store", default="full", choices=["full", "mitm"],
                     help="slice store: full = every slice kept, densities by one streaming pass (fastest on a 180 GB part, the default here); "
