@@ -321,8 +321,8 @@ CL_SEED = 20120454
 
 @pytest.fixture(scope="module")
 def oracle_cfg5s(oracle):
-    """Config 5s (128^3, Ns = 100, q and q+: 200 RQM4 steps) on the oracle, ONCE per session (~2 x 150 s on one core): a full
-    solve (Q, phi_A, phi_B) and the complex-Langevin step from the same fields (which solves again)."""
+    """Config 5s (128^3, Ns = 100, q and q+: 200 RQM4 steps) on the oracle, ONCE per session (~3 x 110 s + 40 s on one core): a
+    full solve (Q, phi_A, phi_B, operators) and the complex-Langevin step from the same fields in both schemes (each solves again)."""
     cfg = inputs.config5(128)
     o = oracle.Oracle(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision="f64", **_kw(cfg))
     o.set_fields(cfg.f0, cfg.f1)
@@ -332,8 +332,11 @@ def oracle_cfg5s(oracle):
     ops = o.operators()                                # H, mu, Pi out of the same solve (Pi: 101 Laplacians, ~40 s)
     o.cl_step(cfg.dt, 0, CL_SEED, 0)
     wp, wm = o.get_fields()
+    o.set_fields(cfg.f0, cfg.f1)
+    o.cl_step(cfg.dt, 1, CL_SEED, 0)                    # the semi-implicit update of Eq. 10-11 from the same fields (one more solve)
+    si = o.get_fields()
     del o
-    return cfg, Q, pa, pb, qN, wp, wm, ops
+    return cfg, Q, pa, pb, qN, wp, wm, ops, si
 
 
 @pytest.mark.parametrize("precision", ["f64", "f32"])
@@ -341,9 +344,9 @@ def test_config5s_full_oracle_solve_and_cl_step(B, oracle_cfg5s, precision):
     """SURVEY 8(d), config 5s through the TMA march in BOTH slice stores - the library default (meet-in-the-middle, densities
     fused into the march) and the full store bench.py times by default (store_both = 1, densities by density_store_kernel):
     Q to 1e-11 (2e-4 in complex64), phi_A, phi_B and q(r,1) element-wise to 1e-9 (2e-4), the fields after one fts_cl_step with
-    identical Philox noise to 1e-9 (2e-4), and - N2 at scale, full store - H, mu and Pi over the 2 x 101 stored slices of 128^3,
-    all against the oracle's full 200-step solve."""
-    cfg, Qo, oa, ob, qN, wpo, wmo, ops_o = oracle_cfg5s
+    identical Philox noise to 1e-9 (2e-4), and - N2 at scale, full store - H, mu and Pi over the 2 x 101 stored slices of 128^3
+    and one semi-implicit step (Eq. 10-11, scheme 1), all against the oracle's full 200-step solves."""
+    cfg, Qo, oa, ob, qN, wpo, wmo, ops_o, si_o = oracle_cfg5s
     dt = torch.complex128 if precision == "f64" else torch.complex64
     tq, tp = (1e-11, 1e-9) if precision == "f64" else (2e-4, 2e-4)
     g = B.Fts(cfg.grid, cfg.cell, cfg.Ns, cfg.model, precision=precision, **_kw(cfg))
@@ -371,6 +374,10 @@ def test_config5s_full_oracle_solve_and_cl_step(B, oracle_cfg5s, precision):
     wp, wm = f.get_fields()
     assert np.max(np.abs(wp.cpu().numpy() - wpo)) <= tp * max(1.0, np.max(np.abs(wpo)))
     assert np.max(np.abs(wm.cpu().numpy() - wmo)) <= tp * max(1.0, np.max(np.abs(wmo)))
+    f.set_fields(_dev(cfg.f0, dt), _dev(cfg.f1, dt))    # N2 at scale: Eq. 10-11 (scheme 1; filter passes at pencil length 128) from the same fields
+    f.cl_step(cfg.dt, 1, CL_SEED, 0)
+    for x, y in zip(f.get_fields(), si_o):
+        assert np.max(np.abs(x.cpu().numpy() - y)) <= tp * max(1.0, np.max(np.abs(y)))
 
 
 @pytest.fixture(scope="module")
