@@ -48,6 +48,24 @@ static fts_status filter3d_t(Ctx* c, void* g, Filt f, cudaStream_t st, const voi
     return FTS_OK;
 }
 
+// The same filter applied to n <= 4 fields in the same five launches (pass_kernel takes one job per blockIdx.y): field i is read
+// from src[i] and its result left in g[i].  Per field the arithmetic is that of filter3d_t, bit for bit.
+template <class T>
+static fts_status filter3d_batch_t(Ctx* c, void* const* g, const void* const* src, int n, Filt f, cudaStream_t st) {
+    PassArgs A; std::memset(&A, 0, sizeof A);
+    for (int i = 0; i < n; ++i) A.job[i] = mkjob(src[i], g[i], OP_FWD);
+    CK(launch_pass<T>(c, 2, A, n, st));
+    for (int i = 0; i < n; ++i) A.job[i] = mkjob(g[i], g[i], OP_FWD);
+    CK(launch_pass<T>(c, 1, A, n, st));
+    for (int i = 0; i < n; ++i) A.job[i] = mkjob(g[i], g[i], OP_FILT);
+    A.filt = f;
+    CK(launch_pass<T>(c, 0, A, n, st));
+    for (int i = 0; i < n; ++i) A.job[i] = mkjob(g[i], g[i], OP_INV);
+    CK(launch_pass<T>(c, 1, A, n, st));
+    CK(launch_pass<T>(c, 2, A, n, st));
+    return FTS_OK;
+}
+
 static fts_status read_scalars(Ctx* c, double* host, int n, cudaStream_t st) {
     int flag = 0;
     CK(cudaMemcpyAsync(host, c->scal, n * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -149,10 +167,17 @@ static fts_status operators_t(Ctx* c, double* Ho, double* muo, double* Pio, cuda
     if (Pio && c->packed) { c->err = "Pi is not available with real_fields"; return FTS_EUNSUPPORTED; }
     if (Pio && c->keep != Ns) { c->err = "Pi needs every slice of q and q+: create the context with store_both = 1"; return FTS_ESTATE; }
     if (Pio) {                                             // K_j = (1/M) sum_x q+_{Ns-j} Laplacian(q_j)
+        // Four slices per set of filter launches (13 launches per four slices instead of 28).  Scratch: G[0], G[1] and the context's
+        // own phi fields, which are temporaries of the step calls (every step recomputes them before use).
         Filt f; f.type = FILT_NEGK2; f.a = 1.0; f.b = f.c = 0.0;
-        for (int j = 0; j <= Ns; ++j) {
-            rc = filter3d_t<T>(c, c->G[0], f, st, q + (size_t)j * M); if (rc) return rc;      // the first pass reads the slice in place
-            CK((reduce<T, RED_PROD>(c, c->G[0], qd + (size_t)(Ns - j) * M, 0.0, 1.0 / (double)M, c->kacc + 2 * j, st)));
+        void* const out[4] = {c->G[0], c->G[1], c->phi[0], c->phi[1]};
+        for (int j0 = 0; j0 <= Ns; j0 += 4) {
+            const int n = Ns + 1 - j0 < 4 ? Ns + 1 - j0 : 4;
+            const void* src[4] = {nullptr, nullptr, nullptr, nullptr};
+            for (int i = 0; i < n; ++i) src[i] = q + (size_t)(j0 + i) * M;                   // the first pass reads the slices in place
+            rc = filter3d_batch_t<T>(c, out, src, n, f, st); if (rc) return rc;
+            for (int i = 0; i < n; ++i)
+                CK((reduce<T, RED_PROD>(c, out[i], qd + (size_t)(Ns - j0 - i) * M, 0.0, 1.0 / (double)M, c->kacc + 2 * (j0 + i), st)));
         }
     }
     if (!c->ops_entry) { rc = field_sums_t<T>(c, st); if (rc) return rc; }      // after fts_cl_step: the sums of its entry fields are already there
